@@ -1,0 +1,117 @@
+/*
+ * gene_nl.h -- C ABI of the B200-native E x B nonlinearity of GENE (flux-tube, pseudo-spectral).
+ *
+ * Operation (sect. 2.1; operator/layout per BASELINE.json north_star):
+ * for every (z, v_par, mu, species) plane p
+ *
+ *     rhs[:, :, p] += scale * N(chi_p, g_p),
+ *     N = dx(chi) * dy(g) - dy(chi) * dx(g)          (the E x B bracket, dealiased by the 3/2 rule)
+ *
+ * i.e. "the fields are preprocessed (... extension ... for dealiasing according to the 3/2-rule)
+ * ..., a fast Fourier transform to real space is applied.  After multiplication the result is
+ * transformed back to the spectral representation, the additional modes are deleted, ... multiplied
+ * with a prefactor, and is finally added to the right-hand side vector", with the
+ * spectral derivatives i*kx, i*ky formed on the device from g and chi (north_star; the paper's
+ * port received them pre-differentiated).  The result equals the truncated spectral
+ * convolution  N(a,b) = sum_{k'+k''=k} (ky' kx'' - kx' ky'') chi(k') g(k'')  up to FP64 rounding.
+ *
+ * Layout (BASELINE.json configs[0]).  All arrays are complex128 (re, im interleaved doubles).
+ *   g, rhs : extents [nx0, nky0, nz, nv, nw, nspec], kx fastest:
+ *            offset(i,j,k,l,m,n) = i + nx0*(j + nky0*(k + nz*(l + nv*(m + nw*n)))).
+ *   chi    : chi_has_v = 0 -> [nx0, nky0, nz, nw, nspec] (no v extent, broadcast over v);
+ *            chi_has_v = 1 -> same extents as g.
+ *   kx of row i: kxmin*i (i < nx0/2), kxmin*(i - nx0) (i > nx0/2).  Row i = nx0/2 (Nyquist) is
+ *   ignored in chi and g and left untouched in rhs.  ky of column j: kymin*j, j = 0..nky0-1; the
+ *   ky < 0 half is implied by reality.  The ky = 0 column should be Hermitian in kx; if it is not,
+ *   its Hermitian part is used (the real part of the synthesis).
+ *   Padded real grid: Nx = 3*nx0/2 by Ny = 3*nky0.
+ *
+ * Everything runs in hand-written sm_100a CUDA kernels in FP64.  There is no CPU fallback, no cuFFT,
+ * no backend dispatch: on a machine without a CUDA device gene_nl_create fails.
+ */
+#ifndef GENE_NL_H
+#define GENE_NL_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gene_nl_plan gene_nl_plan; /* opaque */
+
+/* error codes returned by gene_nl_compute* (0 = success) */
+#define GENE_NL_OK 0
+#define GENE_NL_EINVAL 1       /* NULL / misaligned / overlapping pointer, bad handle            */
+#define GENE_NL_EUNSUPPORTED 2 /* grid size without an instantiated kernel                        */
+#define GENE_NL_ECUDA 3        /* a CUDA runtime call or kernel launch failed                     */
+#define GENE_NL_ENOMEM 4       /* device or pinned-host allocation failed                         */
+
+/*
+ * gene_nl_create -- build a plan on the CURRENT CUDA device (north_star signature).
+ *   nx0   number of kx modes (even; Nx = 3*nx0/2 must be one of 24,48,96,144,192,384,768)
+ *   nky0  number of ky >= 0 modes (Ny = 3*nky0 must be one of 24,48,96,144,192,384)
+ *   nz, nv, nw, nspec   extents of the parametric dimensions (all > 0); planes = nz*nv*nw*nspec
+ *   kxmin, kymin        wavenumber spacings (finite)
+ *   chi_has_v           0: chi has no v extent (shared by the nv planes); 1: chi shaped like g
+ * The plan owns its device tables and scratch (allocated here, freed by gene_nl_destroy).
+ * Returns NULL on failure; gene_nl_last_error() then describes why.
+ */
+gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspec,
+                             double kxmin, double kymin, int chi_has_v);
+
+/*
+ * gene_nl_compute -- rhs += scale * N(chi, g) for all planes.  DEVICE pointers, caller-owned, 16-byte
+ * aligned, layouts as above; chi and g are read-only, rhs must not overlap them.  `stream` is a
+ * cudaStream_t passed as void* (NULL = legacy default stream).  Asynchronous: all work is enqueued on
+ * `stream` and the call returns without synchronising.  One compute may be in flight per plan (the
+ * scratch is shared).  Returns GENE_NL_OK or an error code; on error rhs may be partially updated.
+ */
+int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale,
+                    void* stream);
+
+/*
+ * gene_nl_compute_host -- same operation on HOST buffers (same layouts).  The arrays are streamed
+ * through the device in chunks of planes on several CUDA streams so that host->device copies,
+ * kernels and the device->host copy of rhs overlap ("we split each input array into
+ * (usually four) contiguous chunks of xy-planes, which are transferred and computed in two
+ * asynchronous CUDA streams").  Pinned (page-locked) host memory gives full overlap; pageable memory
+ * works but copies serialise.  SYNCHRONOUS: returns after rhs_host holds the result.
+ */
+int gene_nl_compute_host(gene_nl_plan* h, const void* chi_host, const void* g_host, void* rhs_host,
+                         double scale);
+
+/* gene_nl_destroy -- free the plan's device memory.  NULL is a no-op.  Synchronises the device. */
+void gene_nl_destroy(gene_nl_plan* h);
+
+/* Thread-local description of the last failure in this library ("" if none). */
+const char* gene_nl_last_error(void);
+
+/* Bytes of device scratch + tables owned by the plan. */
+size_t gene_nl_workspace_bytes(const gene_nl_plan* h);
+
+/* Number of kernel launches one gene_nl_compute enqueues (for launch accounting in benchmarks). */
+int gene_nl_launches_per_compute(const gene_nl_plan* h);
+
+/*
+ * gene_nl_query -- plan facts for benchmarks and tests.  `what`:
+ *   0 planes, 1 Nx, 2 Ny, 3 planes per batch, 4 batches per compute,
+ *   5 algorithmic bytes per plane  B = 16*nx0*nky0*(3 + c),
+ *   6 conventional flops per plane F = (3+2c)*T2D + 4M(1+c) + 3NxNy + 4M,
+ *   with c = 1 if chi_has_v else 1/nv.  Returns NaN for an unknown `what` or NULL plan.
+ */
+double gene_nl_query(const gene_nl_plan* h, int what);
+
+/*
+ * gene_nl_probe_peaks -- micro-benchmarks of the two units that bound this path, on the current
+ * device (used by bench.py for the roofline denominators; SURVEY.md 8(d) asks for a measured FP64
+ * peak).  out[0] = FP64 DFMA throughput [TFLOP/s] from independent register-resident FMA chains on
+ * all SMs; out[1] = shared-memory bandwidth [GB/s] from conflict-free 128-bit loads+stores on all
+ * SMs; out[2] = SM clock [MHz] reported by the driver at the end of the probe.  Returns 0 on success.
+ */
+int gene_nl_probe_peaks(double* out3);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GENE_NL_H */

@@ -1,0 +1,431 @@
+// gene_nl.cu -- C ABI (include/gene_nl.h): plan, batching, launch sequence, host streaming driver.
+//
+// One gene_nl_compute walks the phase space in CHUNKS = (w,s) slab x z-range x all v, and inside a
+// chunk in BATCHES of v so that the per-batch scratch (Z, P, Rchi; see nl_kernels.cuh) stays in L2.
+// With chi_has_v = 0 the real-space chi fields of a chunk are formed once and reused by every v
+// (SURVEY.md 7 "chi reuse").  The host entry point streams chunks over several CUDA streams
+// (PAPER.md:69).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/gene_nl.h"
+#include "nl_kernels.cuh"
+
+using gnl::cplx;
+
+namespace {
+
+thread_local std::string g_err;
+
+void set_err(const std::string& s) { g_err = s; }
+
+bool cuda_ok(cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return true;
+    set_err(std::string(what) + ": " + cudaGetErrorString(e));
+    return false;
+}
+
+// ---- per-length kernel tables --------------------------------------------------------------------
+struct XGeom { const cplx* src; cplx* Z; int nky0, nzb; long long vstride; double kxmin, kymin; };
+
+typedef void (*xinv_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double, double);
+typedef void (*xfwd_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double);
+typedef void (*yreal_fn)(const cplx*, cplx*, const cplx*, int);
+typedef void (*ybr_fn)(const cplx*, const cplx*, cplx*, const cplx*, int, int, int);
+
+struct XKernels {
+    int nx, ck, nt;
+    size_t smem_inv, smem_fwd;
+    xinv_fn inv;
+    xfwd_fn fwd;
+};
+struct YKernels {
+    int ny, rp, rt, nt;
+    size_t smem_br, smem_real;
+    ybr_fn br;
+    yreal_fn real;
+};
+
+template <int NX, int A, int B, int CK, int NT>
+XKernels make_x()
+{
+    XKernels k;
+    k.nx = NX; k.ck = CK; k.nt = NT;
+    k.smem_inv = sizeof(cplx) * (size_t)(NX + 2 * CK * gnl::Tile<A, B>::STRIDE);
+    k.smem_fwd = sizeof(cplx) * (size_t)(NX + CK * gnl::Tile<A, B>::STRIDE);
+    k.inv = gnl::k_xinv<NX, A, B, CK, NT>;
+    k.fwd = gnl::k_xfwd<NX, A, B, CK, NT>;
+    return k;
+}
+template <int NY, int A, int B, int RP, int NT>
+YKernels make_y()
+{
+    YKernels k;
+    k.ny = NY; k.rp = RP; k.rt = 2 * RP; k.nt = NT;
+    k.smem_br = sizeof(cplx) * (size_t)(NY + 2 * RP * gnl::Tile<A, B>::STRIDE);
+    k.smem_real = k.smem_br;
+    k.br = gnl::k_ybracket<NY, A, B, RP, NT>;
+    k.real = gnl::k_yreal<NY, A, B, 2 * RP, NT>;
+    return k;
+}
+
+bool find_x(int nx, XKernels* out)
+{
+    switch (nx) {
+    case 24: *out = make_x<24, 3, 8, 8, 128>(); return true;
+    case 48: *out = make_x<48, 6, 8, 8, 128>(); return true;
+    case 96: *out = make_x<96, 12, 8, 8, 128>(); return true;
+    case 144: *out = make_x<144, 12, 12, 8, 128>(); return true;
+    case 192: *out = make_x<192, 24, 8, 8, 128>(); return true;
+    case 384: *out = make_x<384, 24, 16, 4, 128>(); return true;
+    case 768: *out = make_x<768, 24, 32, 4, 128>(); return true;
+    default: return false;
+    }
+}
+// Row pairs per CTA must divide Nx/2; Nx/2 is a multiple of 12 for every supported Nx.
+bool find_y(int ny, YKernels* out)
+{
+    switch (ny) {
+    case 24: *out = make_y<24, 3, 8, 4, 128>(); return true;
+    case 48: *out = make_y<48, 6, 8, 4, 128>(); return true;
+    case 96: *out = make_y<96, 12, 8, 4, 128>(); return true;
+    case 144: *out = make_y<144, 12, 12, 4, 128>(); return true;
+    case 192: *out = make_y<192, 12, 16, 4, 128>(); return true;
+    case 384: *out = make_y<384, 24, 16, 4, 128>(); return true;
+    default: return false;
+    }
+}
+
+struct Scratch {
+    cplx *Z = nullptr, *P = nullptr, *R = nullptr;
+};
+
+struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
+    cudaStream_t stream = nullptr;
+    cplx *g = nullptr, *rhs = nullptr, *chi = nullptr;
+    Scratch scr;
+};
+
+}  // namespace
+
+struct gene_nl_plan {
+    int nx0, nky0, nz, nv, nw, nspec, chi_has_v;
+    double kxmin, kymin;
+    int Nx, Ny;
+    size_t M;       // modes per plane
+    long long planes;
+    int nzb, nvb;   // chunk z-extent and batch v-extent
+    XKernels xk;
+    YKernels yk;
+    cplx *twx = nullptr, *twy = nullptr;
+    Scratch scr;
+    size_t zbytes, pbytes, rbytes;  // per scratch set
+    size_t table_bytes;
+    std::vector<HostStage> stages;  // lazily created by gene_nl_compute_host
+    int device;
+};
+
+namespace {
+
+size_t scratch_budget_bytes()
+{
+    // tuning knob (development): scratch budget per set in MiB; default sized for the 126 MB L2
+    const char* e = getenv("GENE_NL_SCRATCH_MB");
+    long mb = e ? atol(e) : 40;
+    if (mb < 1) mb = 1;
+    return (size_t)mb << 20;
+}
+
+bool alloc_scratch(gene_nl_plan* h, Scratch* s)
+{
+    if (!cuda_ok(cudaMalloc(&s->Z, h->zbytes), "cudaMalloc(Z)")) return false;
+    if (!cuda_ok(cudaMalloc(&s->P, h->pbytes), "cudaMalloc(P)")) return false;
+    if (!cuda_ok(cudaMalloc(&s->R, h->rbytes), "cudaMalloc(Rchi)")) return false;
+    return true;
+}
+void free_scratch(Scratch* s)
+{
+    cudaFree(s->Z); cudaFree(s->P); cudaFree(s->R);
+    s->Z = s->P = s->R = nullptr;
+}
+
+bool upload_twiddles(int n, cplx** out)
+{
+    std::vector<cplx> t(n);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int k = 0; k < n; ++k) {
+        long double ang = two_pi * (long double)k / (long double)n;
+        t[k].x = (double)cosl(ang);
+        t[k].y = (double)sinl(ang);
+    }
+    if (!cuda_ok(cudaMalloc(out, sizeof(cplx) * n), "cudaMalloc(twiddles)")) return false;
+    return cuda_ok(cudaMemcpy(*out, t.data(), sizeof(cplx) * n, cudaMemcpyHostToDevice), "cudaMemcpy(twiddles)");
+}
+
+template <class K>
+bool set_smem(K fn, size_t bytes, const char* name)
+{
+    if (bytes > 227 * 1024) {
+        set_err(std::string(name) + ": shared memory request exceeds 227 KB");
+        return false;
+    }
+    return cuda_ok(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes), name);
+}
+
+// Enqueue one chunk: planes (zi in [0,nzc), vi in [0,nv)), plane offset zi + vstride*vi from g/rhs;
+// chi planes zi (+ cvstride*vi if chi_has_v) from chi.  Returns number of launches or -1.
+int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long cvstride, const cplx* g,
+                  cplx* rhs, long long vstride, int nzc, double scale, cudaStream_t st)
+{
+    const XKernels& xk = h->xk;
+    const YKernels& yk = h->yk;
+    const int xt = h->nky0 / xk.ck;            // column tiles per plane
+    const int yt_pairs = (h->Nx / 2) / yk.rp;  // row-pair tiles per plane
+    const int yt_rows = h->Nx / yk.rt;         // row tiles per plane (k_yreal)
+    const double coef = scale / (2.0 * (double)h->Nx * (double)h->Ny);
+    int launches = 0;
+    if (!h->chi_has_v) {
+        xk.inv<<<nzc * xt, xk.nt, xk.smem_inv, st>>>(chi, s.Z, h->twx, h->nky0, nzc, 0, h->kxmin, h->kymin);
+        yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx);
+        launches += 2;
+    }
+    for (int v0 = 0; v0 < h->nv; v0 += h->nvb) {
+        const int nvc = (h->nv - v0 < h->nvb) ? h->nv - v0 : h->nvb;
+        const int nb = nzc * nvc;
+        const size_t off = (size_t)v0 * (size_t)vstride * h->M;
+        if (h->chi_has_v) {
+            const size_t coff = (size_t)v0 * (size_t)cvstride * h->M;
+            xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(chi + coff, s.Z, h->twx, h->nky0, nzc, cvstride, h->kxmin, h->kymin);
+            yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx);
+            launches += 2;
+        }
+        xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin);
+        yk.br<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, h->chi_has_v);
+        xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef);
+        launches += 3;
+    }
+    if (!cuda_ok(cudaGetLastError(), "kernel launch")) return -1;
+    return launches;
+}
+
+int chunks_per_slab(const gene_nl_plan* h) { return (h->nz + h->nzb - 1) / h->nzb; }
+
+int launches_per_chunk(const gene_nl_plan* h)
+{
+    const int nbatch = (h->nv + h->nvb - 1) / h->nvb;
+    return h->chi_has_v ? 5 * nbatch : 2 + 3 * nbatch;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* gene_nl_last_error(void) { return g_err.c_str(); }
+
+gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspec, double kxmin, double kymin,
+                             int chi_has_v)
+{
+    g_err.clear();
+    if (nx0 <= 0 || nky0 <= 0 || nz <= 0 || nv <= 0 || nw <= 0 || nspec <= 0 || (nx0 & 1) ||
+        !std::isfinite(kxmin) || !std::isfinite(kymin)) {
+        set_err("gene_nl_create: extents must be positive, nx0 even, kxmin/kymin finite");
+        return nullptr;
+    }
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice (no CUDA device: this library has no CPU fallback)")) return nullptr;
+    gene_nl_plan* h = new gene_nl_plan();
+    h->nx0 = nx0; h->nky0 = nky0; h->nz = nz; h->nv = nv; h->nw = nw; h->nspec = nspec;
+    h->chi_has_v = chi_has_v ? 1 : 0;
+    h->kxmin = kxmin; h->kymin = kymin;
+    h->Nx = 3 * nx0 / 2; h->Ny = 3 * nky0;
+    h->M = (size_t)nx0 * nky0;
+    h->planes = (long long)nz * nv * nw * nspec;
+    h->device = dev;
+    if (!find_x(h->Nx, &h->xk) || !find_y(h->Ny, &h->yk)) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "gene_nl_create: unsupported padded grid %dx%d (Nx in {24,48,96,144,192,384,768}, Ny in {24,48,96,144,192,384})", h->Nx, h->Ny);
+        set_err(buf);
+        delete h;
+        return nullptr;
+    }
+    if (nky0 % h->xk.ck || (h->Nx / 2) % h->yk.rp || h->Nx % h->yk.rt) {
+        set_err("gene_nl_create: internal tiling does not divide the grid");
+        delete h;
+        return nullptr;
+    }
+    // batching: chunk = nzb z-planes x all v; batch = nzb x nvb planes with scratch within the budget
+    const size_t W2 = 2 * (size_t)nky0;
+    const size_t zpp = sizeof(cplx) * h->Nx * W2, ppp = zpp / 2, rpp = sizeof(cplx) * (size_t)h->Nx * h->Ny;
+    const size_t budget = scratch_budget_bytes();
+    int nzb = nz;
+    if (!h->chi_has_v) {
+        while (nzb > 1 && (size_t)nzb * rpp > budget / 4) nzb = (nzb + 1) / 2;
+    }
+    const size_t per_plane = zpp + ppp + (h->chi_has_v ? rpp : 0);
+    while (nzb > 1 && (size_t)nzb * per_plane > budget / 2) nzb = (nzb + 1) / 2;
+    const size_t fixed = h->chi_has_v ? 0 : (size_t)nzb * rpp;
+    long long nvb = (long long)((budget > fixed ? budget - fixed : 0) / ((size_t)nzb * per_plane));
+    if (nvb < 1) nvb = 1;
+    if (nvb > nv) nvb = nv;
+    h->nzb = nzb; h->nvb = (int)nvb;
+    const size_t nb = (size_t)nzb * nvb;
+    h->zbytes = zpp * nb;
+    h->pbytes = ppp * nb;
+    h->rbytes = rpp * (h->chi_has_v ? nb : (size_t)nzb);
+    h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
+
+    bool ok = upload_twiddles(h->Nx, &h->twx) && upload_twiddles(h->Ny, &h->twy) && alloc_scratch(h, &h->scr) &&
+              set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
+              set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem");
+    if (!ok) {
+        std::string keep = g_err;
+        gene_nl_destroy(h);
+        g_err = keep;
+        return nullptr;
+    }
+    return h;
+}
+
+void gene_nl_destroy(gene_nl_plan* h)
+{
+    if (!h) return;
+    cudaDeviceSynchronize();
+    for (auto& s : h->stages) {
+        cudaFree(s.g); cudaFree(s.rhs); cudaFree(s.chi);
+        free_scratch(&s.scr);
+        if (s.stream) cudaStreamDestroy(s.stream);
+    }
+    free_scratch(&h->scr);
+    cudaFree(h->twx);
+    cudaFree(h->twy);
+    delete h;
+}
+
+static int check_ptrs(const void* chi, const void* g, void* rhs, size_t gbytes, size_t cbytes)
+{
+    if (!chi || !g || !rhs) { set_err("NULL array pointer"); return GENE_NL_EINVAL; }
+    if (((uintptr_t)chi | (uintptr_t)g | (uintptr_t)rhs) & 15) { set_err("array pointers must be 16-byte aligned"); return GENE_NL_EINVAL; }
+    const char *r0 = (const char*)rhs, *r1 = r0 + gbytes;
+    const char *g0 = (const char*)g, *c0 = (const char*)chi;
+    if ((g0 < r1 && r0 < g0 + gbytes) || (c0 < r1 && r0 < c0 + cbytes)) { set_err("rhs overlaps g or chi"); return GENE_NL_EINVAL; }
+    return GENE_NL_OK;
+}
+
+int gene_nl_compute(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs_, double scale, void* stream)
+{
+    g_err.clear();
+    if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
+    const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
+    int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
+    if (rc) return rc;
+    const cplx* chi = (const cplx*)chi_;
+    const cplx* g = (const cplx*)g_;
+    cplx* rhs = (cplx*)rhs_;
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int ws = 0; ws < h->nw * h->nspec; ++ws) {
+        for (int z0 = 0; z0 < h->nz; z0 += h->nzb) {
+            const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
+            const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * ws) * h->M;
+            const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * ws) * h->M;
+            if (enqueue_chunk(h, h->scr, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, st) < 0)
+                return GENE_NL_ECUDA;
+        }
+    }
+    return GENE_NL_OK;
+}
+
+int gene_nl_compute_host(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs_, double scale)
+{
+    g_err.clear();
+    if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
+    const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
+    int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
+    if (rc) return rc;
+    const size_t pb = sizeof(cplx) * h->M;  // plane bytes
+    const size_t chunk_planes = (size_t)h->nzb * h->nv;
+    if (h->stages.empty()) {
+        const int nstage = 3;
+        h->stages.resize(nstage);
+        for (auto& s : h->stages) {
+            bool ok = cuda_ok(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate") &&
+                      cuda_ok(cudaMalloc(&s.g, chunk_planes * pb), "cudaMalloc(stage g)") &&
+                      cuda_ok(cudaMalloc(&s.rhs, chunk_planes * pb), "cudaMalloc(stage rhs)") &&
+                      cuda_ok(cudaMalloc(&s.chi, (h->chi_has_v ? chunk_planes : (size_t)h->nzb) * pb), "cudaMalloc(stage chi)") &&
+                      alloc_scratch(h, &s.scr);
+            if (!ok) return GENE_NL_ENOMEM;
+        }
+    }
+    const char* chi = (const char*)chi_;
+    const char* g = (const char*)g_;
+    char* rhs = (char*)rhs_;
+    int k = 0;
+    for (int ws = 0; ws < h->nw * h->nspec; ++ws) {
+        for (int z0 = 0; z0 < h->nz; z0 += h->nzb, ++k) {
+            HostStage& s = h->stages[k % h->stages.size()];
+            const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
+            const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * ws) * pb;
+            const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * ws) * pb;
+            // rows = v, width = nzc contiguous planes; host pitch nz planes, staging pitch nzc planes
+            const size_t width = (size_t)nzc * pb, hpitch = (size_t)h->nz * pb;
+            bool ok = cuda_ok(cudaMemcpy2DAsync(s.g, width, g + goff, hpitch, width, h->nv, cudaMemcpyHostToDevice, s.stream), "H2D g") &&
+                      cuda_ok(cudaMemcpy2DAsync(s.rhs, width, rhs + goff, hpitch, width, h->nv, cudaMemcpyHostToDevice, s.stream), "H2D rhs");
+            if (ok) {
+                if (h->chi_has_v)
+                    ok = cuda_ok(cudaMemcpy2DAsync(s.chi, width, chi + coff, hpitch, width, h->nv, cudaMemcpyHostToDevice, s.stream), "H2D chi");
+                else
+                    ok = cuda_ok(cudaMemcpyAsync(s.chi, chi + coff, width, cudaMemcpyHostToDevice, s.stream), "H2D chi");
+            }
+            if (!ok) return GENE_NL_ECUDA;
+            if (enqueue_chunk(h, s.scr, s.chi, nzc, s.g, s.rhs, nzc, nzc, scale, s.stream) < 0) return GENE_NL_ECUDA;
+            if (!cuda_ok(cudaMemcpy2DAsync(rhs + goff, hpitch, s.rhs, width, width, h->nv, cudaMemcpyDeviceToHost, s.stream), "D2H rhs"))
+                return GENE_NL_ECUDA;
+        }
+    }
+    for (auto& s : h->stages)
+        if (!cuda_ok(cudaStreamSynchronize(s.stream), "cudaStreamSynchronize")) return GENE_NL_ECUDA;
+    return GENE_NL_OK;
+}
+
+size_t gene_nl_workspace_bytes(const gene_nl_plan* h)
+{
+    if (!h) return 0;
+    return h->zbytes + h->pbytes + h->rbytes + h->table_bytes;
+}
+
+int gene_nl_launches_per_compute(const gene_nl_plan* h)
+{
+    if (!h) return 0;
+    return h->nw * h->nspec * chunks_per_slab(h) * launches_per_chunk(h);
+}
+
+double gene_nl_query(const gene_nl_plan* h, int what)
+{
+    if (!h) return NAN;
+    const double c = h->chi_has_v ? 1.0 : 1.0 / h->nv;
+    const double M = (double)h->M, Nx = h->Nx, Ny = h->Ny;
+    switch (what) {
+    case 0: return (double)h->planes;
+    case 1: return Nx;
+    case 2: return Ny;
+    case 3: return (double)h->nzb * h->nvb;
+    case 4: return (double)h->nw * h->nspec * chunks_per_slab(h) * ((h->nv + h->nvb - 1) / h->nvb);
+    case 5: return 16.0 * M * (3.0 + c);
+    case 6: {
+        const double t2d = h->nky0 * 5.0 * Nx * std::log2(Nx) + Nx * 2.5 * Ny * std::log2(Ny);
+        return (3.0 + 2.0 * c) * t2d + 4.0 * M * (1.0 + c) + 3.0 * Nx * Ny + 4.0 * M;
+    }
+    default: return NAN;
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,167 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element on the same
+seeded inputs (north_star: max over planes of ||N_gpu - N_ref||_2/||N_ref||_2 <= 1e-11)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from helpers import TOL, check_parity, gpu_compute, oracle_on_planes, plane_errors, sample_planes
+from paper_1310_1485_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(autouse=True)
+def _default_budget(monkeypatch):
+    monkeypatch.delenv("GENE_NL_SCRATCH_MB", raising=False)
+
+
+def test_config0_all_planes_against_oracle_and_definition(cuda_device):
+    wl = W.CONFIGS[0]
+    err = check_parity(wl, cuda_device, backend=oracle.DFT_NAIVE)
+    assert err <= TOL
+    # and directly against the definition (truncated convolution) on every plane
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    out = W.as_planes(gpu_compute(wl, chi, g, rhs), wl).cpu().numpy()
+    X, G = W.as_planes(chi, wl).cpu().numpy(), W.as_planes(g, wl).cpu().numpy()
+    for p in range(wl.planes):
+        N = oracle.nl_convolution_plane(X[W.chi_plane_of(wl, p)], G[p], wl.kxmin, wl.kymin)
+        assert np.linalg.norm(out[p] - wl.scale * N) <= TOL * np.linalg.norm(N)
+
+
+# every instantiated x length (nx0 = 2 Nx / 3) and y length (nky0 = Ny / 3), both chi layouts,
+# extents that do not divide the batch sizes (ragged z / v tails once the budget is squeezed)
+SHAPES = [
+    (16, 8, 3, 5, 2, 1, False), (16, 8, 2, 3, 1, 2, True),
+    (32, 16, 3, 2, 1, 1, False), (64, 32, 2, 3, 1, 1, True),
+    (96, 48, 2, 2, 1, 1, True), (96, 48, 3, 2, 1, 1, False),
+    (128, 32, 3, 3, 1, 1, False), (128, 64, 1, 2, 1, 1, True),
+    (256, 64, 2, 2, 1, 1, False), (32, 128, 1, 3, 1, 1, False),
+    (512, 16, 1, 2, 1, 1, True), (16, 8, 1, 1, 1, 1, False),
+]
+
+
+@pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec,chi_has_v", SHAPES)
+def test_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, nw, nspec, chi_has_v):
+    wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, chi_has_v, seed=nx0 + nky0)
+    check_parity(wl, cuda_device)
+
+
+@pytest.mark.parametrize("budget_mb", ["1", "3"])
+def test_ragged_batches_under_a_tiny_scratch_budget(cuda_device, monkeypatch, budget_mb):
+    monkeypatch.setenv("GENE_NL_SCRATCH_MB", budget_mb)
+    for chi_has_v in (False, True):
+        wl = W.small_workload(64, 32, 5, 7, 2, 1, 0.05, 0.05, chi_has_v, seed=21)
+        check_parity(wl, cuda_device)
+
+
+def test_properties_scale_zero_linearity_antisymmetry(cuda_device):
+    wl = W.small_workload(64, 32, 2, 3, 1, 1, 0.05, 0.05, True, seed=5)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    assert torch.equal(gpu_compute(wl, chi, g, rhs, scale=0.0), rhs)        # scale = 0: bit-identical
+    zero = torch.zeros_like(rhs)
+    n1 = gpu_compute(wl, chi, g, zero, scale=1.0)
+    n2 = gpu_compute(wl, chi, g, zero, scale=-2.5)
+    assert (n2 + 2.5 * n1).abs().max() <= 1e-14 * n1.abs().max()             # linear in scale
+    nswap = gpu_compute(wl, g, chi, zero, scale=1.0)                        # N(g,chi) = -N(chi,g)
+    assert (n1 + nswap).abs().max() <= 1e-13 * n1.abs().max()
+    nself = gpu_compute(wl, g, g, zero, scale=1.0)                          # N(g,g) = 0
+    assert nself.abs().max() <= 1e-13 * n1.abs().max()
+    # deterministic: two runs give the same bits
+    assert torch.equal(n1, gpu_compute(wl, chi, g, zero, scale=1.0))
+
+
+def test_nyquist_rows_of_inputs_are_ignored(cuda_device):
+    wl = W.small_workload(32, 16, 2, 2, 1, 1, 0.1, 0.1, False, seed=6)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    base = gpu_compute(wl, chi, g, rhs)
+    chi2, g2 = chi.clone(), g.clone()
+    chi2[..., wl.nx0 // 2] = 5.0 + 1.0j
+    g2[..., wl.nx0 // 2] = -2.0 + 7.0j
+    assert torch.equal(gpu_compute(wl, chi2, g2, rhs), base)
+
+
+def test_non_hermitian_ky0_column_follows_reading_R7(cuda_device):
+    wl = W.small_workload(32, 16, 1, 2, 1, 1, 0.1, 0.1, True, seed=7)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    gen = torch.Generator(device=cuda_device).manual_seed(1)
+    for t in (chi, g):
+        col = torch.randn(t[..., 0, :].shape + (2,), dtype=torch.float64, device=cuda_device, generator=gen)
+        t[..., 0, :] = torch.view_as_complex(col)
+    out = gpu_compute(wl, chi, g, rhs)
+    planes = np.arange(wl.planes)
+    ref, R, _, _ = oracle_on_planes(wl, chi, g, rhs, planes, backend=oracle.DFT_NAIVE)
+    assert plane_errors(wl, W.as_planes(out, wl).cpu().numpy(), ref, R).max() <= TOL
+
+
+def test_host_entry_point_matches_oracle(cuda_device, monkeypatch):
+    check_parity(W.CONFIGS[0], cuda_device, host=True)
+    monkeypatch.setenv("GENE_NL_SCRATCH_MB", "2")
+    for chi_has_v in (False, True):
+        wl = W.small_workload(64, 32, 5, 3, 2, 2, 0.05, 0.05, chi_has_v, seed=22)
+        check_parity(wl, cuda_device, host=True)
+
+
+def test_errors_are_reported_not_swallowed(cuda_device):
+    from paper_1310_1485_b200 import GeneNL, GeneNLError, gene_nl_create
+    with pytest.raises(GeneNLError):
+        gene_nl_create(20, 8, 1, 1, 1, 1, 0.1, 0.1, 0)      # Nx = 30: no kernel
+    with pytest.raises(GeneNLError):
+        gene_nl_create(16, 7, 1, 1, 1, 1, 0.1, 0.1, 0)      # Ny = 21
+    with pytest.raises(GeneNLError):
+        gene_nl_create(15, 8, 1, 1, 1, 1, 0.1, 0.1, 0)      # odd nx0
+    with pytest.raises(GeneNLError):
+        gene_nl_create(16, 8, 0, 1, 1, 1, 0.1, 0.1, 0)      # empty extent
+    wl = W.CONFIGS[0]
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    with GeneNL(wl) as nl:
+        with pytest.raises(GeneNLError):
+            nl.compute(chi, g, g)                             # rhs overlaps g
+        with pytest.raises(GeneNLError):
+            nl.compute(chi, g, rhs.data_ptr() + 8)            # misaligned
+        with pytest.raises(GeneNLError):
+            nl.compute(0, g, rhs)                             # NULL
+        nl.compute(chi, g, rhs)                               # and the plan still works afterwards
+        torch.cuda.synchronize()
+
+
+def _full_size(cuda_device, idx, nsample):
+    wl = W.CONFIGS[idx]
+    need = 16 * wl.nx0 * wl.nky0 * (3 * wl.planes + wl.chi_planes) * 1.15
+    free, _ = torch.cuda.mem_get_info()
+    if free < need:
+        pytest.skip(f"{wl.name} needs {need / 2**30:.0f} GiB of device memory")
+    return check_parity(wl, cuda_device, nsample=nsample)
+
+
+def test_config1_full_size_sampled_planes(cuda_device):
+    _full_size(cuda_device, 1, 48)
+
+
+def test_config2_full_size_sampled_planes(cuda_device):
+    _full_size(cuda_device, 2, 20)
+
+
+def test_config4_full_size_sampled_planes(cuda_device):
+    _full_size(cuda_device, 4, 24)
+
+
+def test_config3_full_size_sampled_planes(cuda_device):
+    _full_size(cuda_device, 3, 6)
+
+
+def test_config1_sampled_modes_against_the_definition(cuda_device):
+    """Sampled outputs the definition can compute one by one, at BASELINE.json's full size."""
+    wl = W.CONFIGS[1]
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    out = gpu_compute(wl, chi, g, rhs)
+    ii = np.array([0, 1, 63, 65, 127, 17, 100, 40, 5, 90])
+    jj = np.array([0, 31, 5, 0, 31, 16, 1, 30, 0, 12])
+    for p in sample_planes(wl, 6, seed=1):
+        X = W.as_planes(chi, wl)[W.chi_plane_of(wl, int(p))].cpu().numpy()
+        G = W.as_planes(g, wl)[int(p)].cpu().numpy()
+        N = oracle.nl_convolution_modes(X, G, wl.kxmin, wl.kymin, ii, jj)
+        d = (W.as_planes(out, wl)[int(p)] - W.as_planes(rhs, wl)[int(p)]).cpu().numpy()[jj, ii]
+        assert np.abs(d - wl.scale * N).max() <= 1e-11 * np.abs(N).max()
