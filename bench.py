@@ -1,0 +1,337 @@
+#!/usr/bin/env python
+"""bench.py -- E x B nonlinearity planes/s on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py --gpus N --steps K --warmup W [--config 1] [--impl reference]
+
+A "step" is one pass of the whole hot path (gene_nl_compute: derivative + pad + to real space,
+bracket, back, delete modes, prefactor, add to rhs) over all planes of the workload.  At N = 1 the
+workload is BASELINE.json configs[1] (128x32 modes, 8192 planes, 512 MiB per array).  For N > 1
+(torchrun, one rank per GPU) every rank runs its own configs[1]-sized problem (planes are
+independent: weak scaling, no collective on the data path); the time is the max over ranks.
+
+Keys beyond the base contract: `roofline` (dominant kernel, timed live with CUDA events on the
+launching stream through gene_nl_compute_profiled), `roofline_step` (whole step), `kernels`
+(per-class device time), `cpu_baseline` (the oracle on the host cores, bounded sample), `e2e`
+(gene_nl_compute_host on pinned host buffers, copies inside the timed region), `clocks`.
+`--impl reference` times the CPU oracle as it stands (this tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ExB nonlinearity planes/s"
+UNIT = "planes/s"
+# FP64 ALU peak model: 148 SMs x 64 FP64 FMA lanes/SM/clk x 2 flop x 1.965 GHz (DESIGN.md sect. 7)
+FP64_LANES_PER_SM = 64
+
+
+def per_kernel_flops(wl):
+    """Conventional flop split of SURVEY.md 8(d)'s F over the four kernel classes (DESIGN.md sect. 7)."""
+    Nx, Ny, M = wl.Nx, wl.Ny, wl.nx0 * wl.nky0
+    x1 = wl.nky0 * 5.0 * Nx * math.log2(Nx)      # x half of one 2-D transform (nky0 live columns)
+    y1 = Nx * 2.5 * Ny * math.log2(Ny)           # y half of one real 2-D transform
+    P, Q = wl.planes, wl.chi_planes
+    return {
+        "k_xinv": (P + Q) * (2 * x1 + 4 * M),    # derivative (2 mult/value) + two x-syntheses
+        "k_yreal": Q * (2 * y1),                 # two real y-syntheses (dx chi, dy chi)
+        "k_ybracket": P * (3 * y1 + 3 * Nx * Ny),  # two y-syntheses, bracket, one y-analysis
+        "k_xfwd": P * (x1 + 4 * M),              # x-analysis + scale/accumulate (2 FMA/value)
+    }
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, torch_index, period=0.02):
+        super().__init__(daemon=True)
+        self.period, self.samples, self.reasons, self.max_mhz = period, [], set(), None
+        self._halt = threading.Event()
+        self.h = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            uuid = str(torch.cuda.get_device_properties(torch_index).uuid)
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid).encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.h = None
+
+    def run(self):
+        if self.h is None:
+            return
+        while not self._halt.is_set():
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for b, name in self.REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._halt.wait(self.period)
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def time_oracle(wl, seconds, threads):
+    """The oracle as it stands on a bounded sample of the workload (`seconds` of wall time on `threads`
+    cores): returns (planes/s, planes, elapsed)."""
+    import numpy as np
+    import torch
+
+    import oracle
+    from paper_1310_1485_b200 import workloads as W
+
+    # inputs for a slab that contains the sampled planes: one (w,s) slab of the workload's shape
+    sub = W.Workload(wl.name + "_slab", wl.nx0, wl.nky0, wl.nz, wl.nv, 1, 1, wl.kxmin, wl.kymin,
+                     wl.chi_has_v, wl.seed, wl.rhs_random, wl.scale)
+    chi, g, rhs = W.make_inputs(sub, "cpu")
+    G, X, R = (W.as_planes(t, sub).numpy() for t in (g, chi, rhs))
+    ci = np.array([W.chi_plane_of(sub, p) for p in range(sub.planes)])
+
+    def run(n):
+        n = min(n, sub.planes)
+        t0 = time.perf_counter()
+        oracle.nl_pseudospectral(X, G[:n], R[:n], wl.scale, wl.kxmin, wl.kymin, ci[:n])
+        return n, time.perf_counter() - t0
+
+    n, dt = run(threads)                        # calibration: one plane per thread
+    want = int(max(threads, min(sub.planes, n / dt * seconds)))
+    want -= want % threads
+    n, dt = run(max(want, threads))
+    return n / dt, n, dt
+
+
+def reference_arm(args, wl):
+    """`--impl reference`: the CPU oracle, as it stands, on the host cores; rank 0 only."""
+    import oracle
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+
+    from paper_1310_1485_b200 import workloads as W
+    threads = oracle.num_threads()
+    sub = W.Workload(wl.name + "_slab", wl.nx0, wl.nky0, wl.nz, wl.nv, 1, 1, wl.kxmin, wl.kymin,
+                     wl.chi_has_v, wl.seed, wl.rhs_random, wl.scale)
+    chi, g, rhs = W.make_inputs(sub, "cpu")
+    G, X, R = (W.as_planes(t, sub).numpy() for t in (g, chi, rhs))
+    ci = np.array([W.chi_plane_of(sub, p) for p in range(sub.planes)])
+    t0 = time.perf_counter()
+    oracle.nl_pseudospectral(X, G[:threads], R[:threads], wl.scale, wl.kxmin, wl.kymin, ci[:threads])
+    rate = threads / (time.perf_counter() - t0)
+    total_steps = args.steps + args.warmup
+    n = int(min(sub.planes, max(threads, rate * 100.0 / max(total_steps, 1))))
+    n -= n % threads
+    n = max(n, threads)
+    for _ in range(args.warmup):
+        oracle.nl_pseudospectral(X, G[:n], R[:n], wl.scale, wl.kxmin, wl.kymin, ci[:n])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.nl_pseudospectral(X, G[:n], R[:n], wl.scale, wl.kxmin, wl.kymin, ci[:n])
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    sample = f"{n} planes of {wl.name} per step (one (w,s) slab), recursive radix-2/3 FFT oracle"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "planes_per_step": n, "nx0": wl.nx0, "nky0": wl.nky0},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    from paper_1310_1485_b200 import workloads as W
+    wl = W.CONFIGS[args.config]
+    if args.impl == "reference":
+        reference_arm(args, wl)
+        return
+
+    import torch
+
+    from paper_1310_1485_b200 import GeneNL, gene_nl_probe_peaks
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # every rank owns an independent problem of the workload's shape (weak scaling)
+    my = W.Workload(wl.name, wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin,
+                    wl.chi_has_v, wl.seed + 1000 * rank, wl.rhs_random, wl.scale)
+    chi, g, rhs = W.make_inputs(my, dev)
+    nl = GeneNL(my)
+    stream = torch.cuda.current_stream()
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
+        nl.compute(chi, g, rhs, stream=stream)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        nl.compute(chi, g, rhs, stream=stream)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_total = float(ms.item())
+    ms_per_step = ms_total / args.steps
+    planes_total = my.planes * world
+    value = planes_total / (ms_per_step * 1e-3)
+
+    # per-kernel device time, live, with CUDA events on the launching stream
+    prof_ms = {k: 0.0 for k in ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd")}
+    prof_n = dict.fromkeys(prof_ms, 0)
+    nprof = 3
+    for _ in range(nprof):
+        m, n = nl.compute_profiled(chi, g, rhs, stream=stream)
+        for k in prof_ms:
+            prof_ms[k] += m[k]
+            prof_n[k] += n[k]
+    flops = per_kernel_flops(my)
+    fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    try:
+        probe_tf, probe_smem_gbs, _ = gene_nl_probe_peaks()
+    except Exception:
+        probe_tf, probe_smem_gbs = None, None
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    kernels = {}
+    for k in prof_ms:
+        if prof_n[k]:
+            avg_ms = prof_ms[k] / prof_n[k]
+            kernels[k] = {"launches_per_step": prof_n[k] // nprof, "ms_per_step": prof_ms[k] / nprof,
+                          "avg_launch_us": 1e3 * avg_ms,
+                          "tflops": flops[k] * nprof / (prof_ms[k] * 1e-3) / 1e12}
+    dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
+    traffic = None
+    try:  # measured DRAM bytes per launch of the dominant kernel, from the committed ncu capture
+        t = json.load(open(os.path.join(ROOT, "profiles", "dram_traffic.json")))
+        traffic = t.get(wl.name, {}).get(dom)
+    except Exception:
+        pass
+    roofline = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
+                "unit": "TFLOP/s", "frac": kernels[dom]["tflops"] / fp64_model, "traffic": traffic,
+                "peak_source": "model 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md sect. 7)",
+                "peak_measured_dfma": probe_tf, "smem_gbs_measured": probe_smem_gbs,
+                "share_of_step": kernels[dom]["ms_per_step"] / sum(v["ms_per_step"] for v in kernels.values())}
+    F, B = nl.query(6), nl.query(5)
+    step_tf = F * my.planes / (ms_per_step * 1e-3) / 1e12
+    step_gbs = B * my.planes / (ms_per_step * 1e-3) / 1e9
+    t_alu, t_hbm = F / (fp64_model * 1e12), B / (hbm_peak * 1e9)
+    roof_planes = 1.0 / max(t_alu, t_hbm)
+    roofline_step = {"bound": "alu" if t_alu >= t_hbm else "hbm", "achieved_tflops": step_tf,
+                     "achieved_hbm_gbs": step_gbs, "peak_tflops": fp64_model, "peak_hbm_gbs": hbm_peak,
+                     "roofline_planes_per_s": roof_planes, "frac": (value / world) / roof_planes,
+                     "flops_per_plane": F, "bytes_per_plane": B}
+
+    # end to end through the host entry point: pinned host buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hchi, hg, hrhs = (t.cpu().pin_memory() for t in (chi, g, rhs))
+        nl.compute_host(hchi, hg, hrhs)   # warm-up (allocates staging)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            nl.compute_host(hchi, hg, hrhs)
+        torch.cuda.synchronize()
+        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        gb = my.plane_bytes * my.planes
+        e2e = {"value": planes_total * args.e2e_steps / float(dt.item()), "unit": UNIT,
+               "h2d_bytes_per_step": 2 * gb + my.plane_bytes * my.chi_planes, "d2h_bytes_per_step": gb,
+               "steps": args.e2e_steps, "api": "gene_nl_compute_host (pinned host buffers)"}
+        del hchi, hg, hrhs
+
+    launches = nl.launches_per_compute * args.steps
+    nl.close()
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        threads = oracle.num_threads()
+        v, n, dt = time_oracle(wl, args.cpu_seconds / max(threads, 1), threads)
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": f"{n} planes of {wl.name} (first planes of one (w,s) slab), {dt:.1f} s wall"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": my.planes,
+                       "padded_grid": [wl.Nx, wl.Ny], "chi_has_v": wl.chi_has_v,
+                       "cache": "inputs larger than L2 (g+rhs+chi = %.0f MiB per GPU)" %
+                                ((2 * my.planes + my.chi_planes) * my.plane_bytes / 2 ** 20),
+                       "parallelism": f"planes x{world} (independent problems per GPU)"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
+            "roofline": roofline, "roofline_step": roofline_step, "kernels": kernels,
+            "cpu_baseline": cpu_baseline,
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

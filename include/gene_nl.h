@@ -71,6 +71,16 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, 
                     void* stream);
 
 /*
+ * gene_nl_compute_profiled -- gene_nl_compute with a CUDA-event pair recorded on `stream` around every
+ * kernel launch, then a stream synchronise.  ms4[c] receives the summed device time [ms] and
+ * launches4[c] the launch count of kernel class c: 0 = x-synthesis (derivative + pad + x half of the
+ * transform to real space), 1 = chi real-space fields, 2 = y-synthesis + bracket + y-analysis,
+ * 3 = x-analysis + delete modes + prefactor + add to rhs.  Used by bench.py for per-kernel rooflines.
+ */
+int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale,
+                             void* stream, double* ms4, int* launches4);
+
+/*
  * gene_nl_compute_host -- same operation on HOST buffers (same layouts).  The arrays are streamed
  * through the device in chunks of planes on several CUDA streams so that host->device copies,
  * kernels and the device->host copy of rhs overlap ("we split each input array into

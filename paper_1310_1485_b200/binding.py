@@ -17,7 +17,8 @@ GENE_NL_OK, GENE_NL_EINVAL, GENE_NL_EUNSUPPORTED, GENE_NL_ECUDA, GENE_NL_ENOMEM 
 
 # every symbol include/gene_nl.h declares
 EXPORTED_SYMBOLS = (
-    "gene_nl_create", "gene_nl_compute", "gene_nl_compute_host", "gene_nl_destroy", "gene_nl_last_error",
+    "gene_nl_create", "gene_nl_compute", "gene_nl_compute_profiled", "gene_nl_compute_host", "gene_nl_destroy",
+    "gene_nl_last_error",
     "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query", "gene_nl_probe_peaks",
 )
 
@@ -48,6 +49,8 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_create.restype = vp
         lib.gene_nl_compute.argtypes = [vp, vp, vp, vp, dbl, vp]
         lib.gene_nl_compute.restype = i
+        lib.gene_nl_compute_profiled.argtypes = [vp, vp, vp, vp, dbl, vp, ctypes.POINTER(dbl), ctypes.POINTER(i)]
+        lib.gene_nl_compute_profiled.restype = i
         lib.gene_nl_compute_host.argtypes = [vp, vp, vp, vp, dbl]
         lib.gene_nl_compute_host.restype = i
         lib.gene_nl_destroy.argtypes = [vp]
@@ -98,6 +101,25 @@ def gene_nl_compute(h, chi, g, rhs, scale, stream=None) -> None:
         raise GeneNLError(f"gene_nl_compute failed ({rc}): {gene_nl_last_error()}")
 
 
+KERNEL_CLASSES = ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd")
+
+
+def gene_nl_compute_profiled(h, chi, g, rhs, scale, stream=None):
+    """gene_nl_compute with per-launch CUDA events; returns ({class: ms}, {class: launches}); synchronises."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    ms = (ctypes.c_double * 4)()
+    n = (ctypes.c_int * 4)()
+    rc = load_library().gene_nl_compute_profiled(h, _ptr(chi), _ptr(g), _ptr(rhs), float(scale),
+                                                 int(stream) or None, ms, n)
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_compute_profiled failed ({rc}): {gene_nl_last_error()}")
+    return dict(zip(KERNEL_CLASSES, map(float, ms))), dict(zip(KERNEL_CLASSES, map(int, n)))
+
+
 def gene_nl_compute_host(h, chi, g, rhs, scale) -> None:
     """Same on HOST arrays (torch CPU tensors, ideally pinned, or raw addresses); synchronous."""
     rc = load_library().gene_nl_compute_host(h, _ptr(chi), _ptr(g), _ptr(rhs), float(scale))
@@ -140,6 +162,9 @@ class GeneNL:
 
     def compute(self, chi, g, rhs, scale=None, stream=None):
         gene_nl_compute(self.h, chi, g, rhs, self.wl.scale if scale is None else scale, stream)
+
+    def compute_profiled(self, chi, g, rhs, scale=None, stream=None):
+        return gene_nl_compute_profiled(self.h, chi, g, rhs, self.wl.scale if scale is None else scale, stream)
 
     def compute_host(self, chi, g, rhs, scale=None):
         gene_nl_compute_host(self.h, chi, g, rhs, self.wl.scale if scale is None else scale)

@@ -108,6 +108,31 @@ struct Scratch {
     cplx *Z = nullptr, *P = nullptr, *R = nullptr;
 };
 
+// Optional per-launch CUDA-event timing (gene_nl_compute_profiled): kernel classes
+enum { K_XINV = 0, K_YREAL = 1, K_YBRACKET = 2, K_XFWD = 3, K_CLASSES = 4 };
+struct Profiler {
+    cudaStream_t st;
+    std::vector<cudaEvent_t> ev;  // pairs (before, after)
+    std::vector<int> cls;
+    cudaEvent_t begin(int c)
+    {
+        cudaEvent_t a, b;
+        cudaEventCreate(&a);
+        cudaEventCreate(&b);
+        ev.push_back(a);
+        ev.push_back(b);
+        cls.push_back(c);
+        cudaEventRecord(a, st);
+        return b;
+    }
+};
+#define GNL_LAUNCH(prof, c, call)                          \
+    do {                                                    \
+        cudaEvent_t e_ = (prof) ? (prof)->begin(c) : nullptr; \
+        call;                                               \
+        if (prof) cudaEventRecord(e_, (prof)->st);          \
+    } while (0)
+
 struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
     cudaStream_t stream = nullptr;
     cplx *g = nullptr, *rhs = nullptr, *chi = nullptr;
@@ -183,7 +208,7 @@ bool set_smem(K fn, size_t bytes, const char* name)
 // Enqueue one chunk: planes (zi in [0,nzc), vi in [0,nv)), plane offset zi + vstride*vi from g/rhs;
 // chi planes zi (+ cvstride*vi if chi_has_v) from chi.  Returns number of launches or -1.
 int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long cvstride, const cplx* g,
-                  cplx* rhs, long long vstride, int nzc, double scale, cudaStream_t st)
+                  cplx* rhs, long long vstride, int nzc, double scale, cudaStream_t st, Profiler* prof = nullptr)
 {
     const XKernels& xk = h->xk;
     const YKernels& yk = h->yk;
@@ -193,8 +218,8 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
     const double coef = scale / (2.0 * (double)h->Nx * (double)h->Ny);
     int launches = 0;
     if (!h->chi_has_v) {
-        xk.inv<<<nzc * xt, xk.nt, xk.smem_inv, st>>>(chi, s.Z, h->twx, h->nky0, nzc, 0, h->kxmin, h->kymin);
-        yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx);
+        GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nzc * xt, xk.nt, xk.smem_inv, st>>>(chi, s.Z, h->twx, h->nky0, nzc, 0, h->kxmin, h->kymin)));
+        GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx)));
         launches += 2;
     }
     for (int v0 = 0; v0 < h->nv; v0 += h->nvb) {
@@ -203,13 +228,13 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
         const size_t off = (size_t)v0 * (size_t)vstride * h->M;
         if (h->chi_has_v) {
             const size_t coff = (size_t)v0 * (size_t)cvstride * h->M;
-            xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(chi + coff, s.Z, h->twx, h->nky0, nzc, cvstride, h->kxmin, h->kymin);
-            yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx);
+            GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(chi + coff, s.Z, h->twx, h->nky0, nzc, cvstride, h->kxmin, h->kymin)));
+            GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx)));
             launches += 2;
         }
-        xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin);
-        yk.br<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, h->chi_has_v);
-        xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef);
+        GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin)));
+        GNL_LAUNCH(prof, K_YBRACKET, (yk.br<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, h->chi_has_v)));
+        GNL_LAUNCH(prof, K_XFWD, (xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef)));
         launches += 3;
     }
     if (!cuda_ok(cudaGetLastError(), "kernel launch")) return -1;
@@ -319,7 +344,8 @@ static int check_ptrs(const void* chi, const void* g, void* rhs, size_t gbytes, 
     return GENE_NL_OK;
 }
 
-int gene_nl_compute(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs_, double scale, void* stream)
+static int compute_impl(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs_, double scale, void* stream,
+                        Profiler* prof)
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
@@ -336,11 +362,38 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs
             const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
             const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * ws) * h->M;
             const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * ws) * h->M;
-            if (enqueue_chunk(h, h->scr, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, st) < 0)
+            if (prof) prof->st = st;
+            if (enqueue_chunk(h, h->scr, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, st, prof) < 0)
                 return GENE_NL_ECUDA;
         }
     }
     return GENE_NL_OK;
+}
+
+int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale, void* stream)
+{
+    return compute_impl(h, chi, g, rhs, scale, stream, nullptr);
+}
+
+int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale, void* stream,
+                             double* ms4, int* launches4)
+{
+    if (!ms4 || !launches4) { set_err("NULL output pointer"); return GENE_NL_EINVAL; }
+    Profiler prof;
+    prof.st = (cudaStream_t)stream;
+    int rc = compute_impl(h, chi, g, rhs, scale, stream, &prof);
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    for (int c = 0; c < K_CLASSES; ++c) { ms4[c] = 0.0; launches4[c] = 0; }
+    for (size_t i = 0; i < prof.cls.size(); ++i) {
+        float ms = 0.f;
+        if (e == cudaSuccess && cudaEventElapsedTime(&ms, prof.ev[2 * i], prof.ev[2 * i + 1]) == cudaSuccess) {
+            ms4[prof.cls[i]] += ms;
+            launches4[prof.cls[i]] += 1;
+        }
+    }
+    for (auto ev : prof.ev) cudaEventDestroy(ev);
+    if (rc) return rc;
+    return cuda_ok(e, "cudaStreamSynchronize") ? GENE_NL_OK : GENE_NL_ECUDA;
 }
 
 int gene_nl_compute_host(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs_, double scale)

@@ -148,3 +148,24 @@ def chi_plane_of(wl: Workload, p):
 def as_planes(t: torch.Tensor, wl: Workload) -> torch.Tensor:
     """View an array as (planes, nky0, nx0)."""
     return t.view(-1, wl.nky0, wl.nx0)
+
+
+def shard_slabs(wl: Workload, rank: int, world: int):
+    """Contiguous range [s0, s1) of the nw*nspec (w,s) slabs owned by `rank`: g, rhs AND
+    chi shard together along the slowest indices, so the bracket needs no exchange between ranks."""
+    nslab = wl.nw * wl.nspec
+    base, extra = divmod(nslab, world)
+    s0 = rank * base + min(rank, extra)
+    return s0, s0 + base + (1 if rank < extra else 0)
+
+
+def shard_arrays(wl: Workload, chi, g, rhs, rank: int, world: int):
+    """(sub-workload, chi, g, rhs views) of one rank's slabs; the sub-workload has nw = slabs, nspec = 1."""
+    s0, s1 = shard_slabs(wl, rank, world)
+    n = s1 - s0
+    sub = Workload(f"{wl.name}_rank{rank}of{world}", wl.nx0, wl.nky0, wl.nz, wl.nv, max(n, 0), 1,
+                   wl.kxmin, wl.kymin, wl.chi_has_v, wl.seed, wl.rhs_random, wl.scale)
+    gs = g.reshape((wl.nw * wl.nspec,) + wl.g_shape[2:])[s0:s1]
+    rs = rhs.reshape((wl.nw * wl.nspec,) + wl.g_shape[2:])[s0:s1]
+    cs = chi.reshape((wl.nw * wl.nspec,) + wl.chi_shape[2:])[s0:s1]
+    return sub, cs, gs, rs
