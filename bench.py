@@ -35,18 +35,23 @@ UNIT = "planes/s"
 FP64_LANES_PER_SM = 64
 
 
-def per_kernel_flops(wl):
+def per_kernel_flops(wl, fused=False):
     """Conventional flop split of SURVEY.md 8(d)'s F over the four kernel classes (DESIGN.md sect. 7)."""
     Nx, Ny, M = wl.Nx, wl.Ny, wl.nx0 * wl.nky0
     x1 = wl.nky0 * 5.0 * Nx * math.log2(Nx)      # x half of one 2-D transform (nky0 live columns)
     y1 = Nx * 2.5 * Ny * math.log2(Ny)           # y half of one real 2-D transform
     P, Q = wl.planes, wl.chi_planes
-    return {
-        "k_xinv": (P + Q) * (2 * x1 + 4 * M),    # derivative (2 mult/value) + two x-syntheses
-        "k_yreal": Q * (2 * y1),                 # two real y-syntheses (dx chi, dy chi)
-        "k_ybracket": P * (3 * y1 + 3 * Nx * Ny),  # two y-syntheses, bracket, one y-analysis
-        "k_xfwd": P * (x1 + 4 * M),              # x-analysis + scale/accumulate (2 FMA/value)
+    per_plane = {
+        "k_xinv": 2 * x1 + 4 * M,                # derivative (2 mult/value) + two x-syntheses
+        "k_yreal": 2 * y1,                       # two real y-syntheses (dx chi, dy chi)
+        "k_ybracket": 3 * y1 + 3 * Nx * Ny,      # two y-syntheses, bracket, one y-analysis
+        "k_xfwd": x1 + 4 * M,                    # x-analysis + scale/accumulate (2 FMA/value)
     }
+    if fused:  # the g side of a plane runs in one kernel; k_xinv / k_yreal only see chi
+        return {"k_xinv": Q * per_plane["k_xinv"], "k_yreal": Q * per_plane["k_yreal"],
+                "k_plane_fused": P * (per_plane["k_xinv"] + per_plane["k_ybracket"] + per_plane["k_xfwd"])}
+    return {"k_xinv": (P + Q) * per_plane["k_xinv"], "k_yreal": Q * per_plane["k_yreal"],
+            "k_ybracket": P * per_plane["k_ybracket"], "k_xfwd": P * per_plane["k_xfwd"]}
 
 
 class ClockSampler(threading.Thread):
@@ -235,7 +240,8 @@ def main():
     value = planes_total / (ms_per_step * 1e-3)
 
     # per-kernel device time, live, with CUDA events on the launching stream
-    prof_ms = {k: 0.0 for k in ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd")}
+    from paper_1310_1485_b200.binding import KERNEL_CLASSES
+    prof_ms = {k: 0.0 for k in KERNEL_CLASSES}
     prof_n = dict.fromkeys(prof_ms, 0)
     nprof = 3
     for _ in range(nprof):
@@ -243,7 +249,7 @@ def main():
         for k in prof_ms:
             prof_ms[k] += m[k]
             prof_n[k] += n[k]
-    flops = per_kernel_flops(my)
+    flops = per_kernel_flops(my, fused=nl.query(7) == 1.0)
     fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
     try:
         probe_tf, probe_smem_gbs, _ = gene_nl_probe_peaks()

@@ -72,18 +72,24 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, 
 
 /*
  * gene_nl_compute_profiled -- gene_nl_compute with a CUDA-event pair recorded on `stream` around every
- * kernel launch, then a stream synchronise.  ms4[c] receives the summed device time [ms] and
- * launches4[c] the launch count of kernel class c: 0 = x-synthesis (derivative + pad + x half of the
- * transform to real space), 1 = chi real-space fields, 2 = y-synthesis + bracket + y-analysis,
- * 3 = x-analysis + delete modes + prefactor + add to rhs.  Used by bench.py for per-kernel rooflines.
+ * kernel launch, then a stream synchronise.  ms[c] receives the summed device time [ms] and
+ * launches[c] the launch count of kernel class c (arrays of GENE_NL_KERNEL_CLASSES entries):
+ *   0 k_xinv       x-synthesis: derivative + pad + x half of the transform to real space
+ *   1 k_yreal      chi real-space fields (dx chi, dy chi)
+ *   2 k_ybracket   y-synthesis + bracket + y-analysis           (batched path, large planes)
+ *   3 k_xfwd       x-analysis + delete modes + prefactor + add  (batched path, large planes)
+ *   4 k_plane_fused  the whole g-side of a plane in one persistent kernel, x<->y hand-over in shared
+ *                  memory (planes with Nx <= 192 and Ny <= 96)
+ * Used by bench.py for per-kernel rooflines.
  */
+#define GENE_NL_KERNEL_CLASSES 5
 int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale,
-                             void* stream, double* ms4, int* launches4);
+                             void* stream, double* ms, int* launches);
 
 /*
  * gene_nl_compute_host -- same operation on HOST buffers (same layouts).  The arrays are streamed
- * through the device in chunks of planes on several CUDA streams so that host->device copies,
- * kernels and the device->host copy of rhs overlap ("we split each input array into
+ * through the device in chunks of planes on several CUDA streams (one (w,s) slab each) so that host->device
+ * copies, kernels and the device->host copy of rhs overlap ("we split each input array into
  * (usually four) contiguous chunks of xy-planes, which are transferred and computed in two
  * asynchronous CUDA streams").  Pinned (page-locked) host memory gives full overlap; pageable memory
  * works but copies serialise.  SYNCHRONOUS: returns after rhs_host holds the result.
@@ -108,7 +114,8 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
  *   0 planes, 1 Nx, 2 Ny, 3 planes per batch, 4 batches per compute,
  *   5 algorithmic bytes per plane  B = 16*nx0*nky0*(3 + c),
  *   6 conventional flops per plane F = (3+2c)*T2D + 4M(1+c) + 3NxNy + 4M,
- *   with c = 1 if chi_has_v else 1/nv.  Returns NaN for an unknown `what` or NULL plan.
+ *   with c = 1 if chi_has_v else 1/nv; 7: 1 if the fused shared-memory kernel is used, else 0.
+ *   Returns NaN for an unknown `what` or NULL plan.
  */
 double gene_nl_query(const gene_nl_plan* h, int what);
 

@@ -101,7 +101,7 @@ def gene_nl_compute(h, chi, g, rhs, scale, stream=None) -> None:
         raise GeneNLError(f"gene_nl_compute failed ({rc}): {gene_nl_last_error()}")
 
 
-KERNEL_CLASSES = ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd")
+KERNEL_CLASSES = ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd", "k_plane_fused")
 
 
 def gene_nl_compute_profiled(h, chi, g, rhs, scale, stream=None):
@@ -111,8 +111,8 @@ def gene_nl_compute_profiled(h, chi, g, rhs, scale, stream=None):
         stream = torch.cuda.current_stream().cuda_stream
     elif hasattr(stream, "cuda_stream"):
         stream = stream.cuda_stream
-    ms = (ctypes.c_double * 4)()
-    n = (ctypes.c_int * 4)()
+    ms = (ctypes.c_double * len(KERNEL_CLASSES))()
+    n = (ctypes.c_int * len(KERNEL_CLASSES))()
     rc = load_library().gene_nl_compute_profiled(h, _ptr(chi), _ptr(g), _ptr(rhs), float(scale),
                                                  int(stream) or None, ms, n)
     if rc != GENE_NL_OK:

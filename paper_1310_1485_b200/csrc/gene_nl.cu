@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "../../include/gene_nl.h"
+#include "nl_fused.cuh"
 #include "nl_kernels.cuh"
 
 using gnl::cplx;
@@ -40,6 +41,40 @@ typedef void (*xinv_fn)(const cplx*, cplx*, const cplx*, int, int, long long, do
 typedef void (*xfwd_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double);
 typedef void (*yreal_fn)(const cplx*, cplx*, const cplx*, int);
 typedef void (*ybr_fn)(const cplx*, const cplx*, cplx*, const cplx*, int, int, int);
+typedef void (*fused_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, int, double, double,
+                         double);
+
+struct FusedKernel {
+    fused_fn fn = nullptr;
+    size_t smem = 0;
+    int nt = 0;
+};
+
+template <int AX, int AY, int NW>
+FusedKernel make_fused()
+{
+    FusedKernel k;
+    k.fn = gnl::k_plane_fused<AX, AY, NW>;
+    k.smem = gnl::Fused<AX, AY, NW>::SMEM_BYTES;
+    k.nt = NW * 32;
+    return k;
+}
+
+// Planes whose half-transformed form fits in shared memory (Nx = 8 AX <= 192, Ny = 8 AY <= 96).
+bool find_fused(int nx, int ny, FusedKernel* out)
+{
+    const int key = nx * 1000 + ny;
+    switch (key) {
+#define GNL_FUSED_CASE(AX, AY) case (8 * AX) * 1000 + 8 * AY: *out = make_fused<AX, AY, 8>(); break;
+        GNL_FUSED_CASE(3, 3) GNL_FUSED_CASE(3, 6) GNL_FUSED_CASE(3, 12)
+        GNL_FUSED_CASE(6, 3) GNL_FUSED_CASE(6, 6) GNL_FUSED_CASE(6, 12)
+        GNL_FUSED_CASE(12, 3) GNL_FUSED_CASE(12, 6) GNL_FUSED_CASE(12, 12)
+        GNL_FUSED_CASE(24, 3) GNL_FUSED_CASE(24, 6) GNL_FUSED_CASE(24, 12)
+#undef GNL_FUSED_CASE
+    default: return false;
+    }
+    return out->smem <= 227 * 1024;
+}
 
 struct XKernels {
     int nx, ck, nt;
@@ -59,8 +94,8 @@ XKernels make_x()
 {
     XKernels k;
     k.nx = NX; k.ck = CK; k.nt = NT;
-    k.smem_inv = sizeof(cplx) * (size_t)(NX + 2 * CK * gnl::Tile<A, B>::STRIDE);
-    k.smem_fwd = sizeof(cplx) * (size_t)(NX + CK * gnl::Tile<A, B>::STRIDE);
+    k.smem_inv = sizeof(cplx) * (size_t)(A * gnl::Tile<A, B>::BP + 2 * CK * gnl::Tile<A, B>::STRIDE);
+    k.smem_fwd = sizeof(cplx) * (size_t)(A * gnl::Tile<A, B>::BP + CK * gnl::Tile<A, B>::STRIDE);
     k.inv = gnl::k_xinv<NX, A, B, CK, NT>;
     k.fwd = gnl::k_xfwd<NX, A, B, CK, NT>;
     return k;
@@ -70,7 +105,7 @@ YKernels make_y()
 {
     YKernels k;
     k.ny = NY; k.rp = RP; k.rt = 2 * RP; k.nt = NT;
-    k.smem_br = sizeof(cplx) * (size_t)(NY + 2 * RP * gnl::Tile<A, B>::STRIDE);
+    k.smem_br = sizeof(cplx) * (size_t)((1 + 2 * RP) * gnl::Tile<A, B>::FLAT);
     k.smem_real = k.smem_br;
     k.br = gnl::k_ybracket<NY, A, B, RP, NT>;
     k.real = gnl::k_yreal<NY, A, B, 2 * RP, NT>;
@@ -91,15 +126,16 @@ bool find_x(int nx, XKernels* out)
     }
 }
 // Row pairs per CTA must divide Nx/2; Nx/2 is a multiple of 12 for every supported Nx.
-bool find_y(int ny, YKernels* out)
+bool find_y(int ny, int nx, YKernels* out)
 {
+    const bool rp8 = (nx / 2) % 8 == 0;  // 8 row pairs per CTA when they divide Nx/2, else 4
     switch (ny) {
-    case 24: *out = make_y<24, 3, 8, 4, 128>(); return true;
-    case 48: *out = make_y<48, 6, 8, 4, 128>(); return true;
-    case 96: *out = make_y<96, 12, 8, 4, 128>(); return true;
-    case 144: *out = make_y<144, 12, 12, 4, 128>(); return true;
-    case 192: *out = make_y<192, 12, 16, 4, 128>(); return true;
-    case 384: *out = make_y<384, 24, 16, 4, 128>(); return true;
+    case 24: *out = rp8 ? make_y<24, 3, 8, 8, 64>() : make_y<24, 3, 8, 4, 64>(); return true;
+    case 48: *out = rp8 ? make_y<48, 6, 8, 8, 64>() : make_y<48, 6, 8, 4, 64>(); return true;
+    case 96: *out = rp8 ? make_y<96, 12, 8, 8, 64>() : make_y<96, 12, 8, 4, 64>(); return true;
+    case 144: *out = rp8 ? make_y<144, 12, 12, 8, 96>() : make_y<144, 12, 12, 4, 96>(); return true;
+    case 192: *out = make_y<192, 12, 16, 4, 64>(); return true;
+    case 384: *out = make_y<384, 24, 16, 4, 64>(); return true;
     default: return false;
     }
 }
@@ -109,7 +145,7 @@ struct Scratch {
 };
 
 // Optional per-launch CUDA-event timing (gene_nl_compute_profiled): kernel classes
-enum { K_XINV = 0, K_YREAL = 1, K_YBRACKET = 2, K_XFWD = 3, K_CLASSES = 4 };
+enum { K_XINV = 0, K_YREAL = 1, K_YBRACKET = 2, K_XFWD = 3, K_FUSED = 4, K_CLASSES = 5 };
 struct Profiler {
     cudaStream_t st;
     std::vector<cudaEvent_t> ev;  // pairs (before, after)
@@ -150,6 +186,11 @@ struct gene_nl_plan {
     int nzb, nvb;   // chunk z-extent and batch v-extent
     XKernels xk;
     YKernels yk;
+    FusedKernel fk;
+    bool fused = false;
+    int fused_grid = 0;
+    int nss = 1;      // fused: (w,s) slabs per launch (Rchi of that many slabs is kept)
+    long long nbz = 1;  // fused: chi planes per k_xinv/k_yreal batch
     cplx *twx = nullptr, *twy = nullptr;
     Scratch scr;
     size_t zbytes, pbytes, rbytes;  // per scratch set
@@ -164,7 +205,7 @@ size_t scratch_budget_bytes()
 {
     // tuning knob (development): scratch budget per set in MiB; default sized for the 126 MB L2
     const char* e = getenv("GENE_NL_SCRATCH_MB");
-    long mb = e ? atol(e) : 40;
+    long mb = e ? atol(e) : 192;
     if (mb < 1) mb = 1;
     return (size_t)mb << 20;
 }
@@ -241,6 +282,49 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
     return launches;
 }
 
+// Enqueue `nslab` contiguous (w,s) slabs (standard strides: v stride nz planes).  Returns launches or -1.
+int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx* g, cplx* rhs, int nslab,
+                  double scale, cudaStream_t st, Profiler* prof = nullptr)
+{
+    int launches = 0;
+    if (h->fused) {
+        const XKernels& xk = h->xk;
+        const YKernels& yk = h->yk;
+        const int xt = h->nky0 / xk.ck, yt_rows = h->Nx / yk.rt;
+        const double coef = scale / (2.0 * (double)h->Nx * (double)h->Ny);
+        for (int s0 = 0; s0 < nslab; s0 += h->nss) {
+            const int ns = (nslab - s0 < h->nss) ? nslab - s0 : h->nss;
+            const size_t cps = (size_t)h->nz * (h->chi_has_v ? h->nv : 1);  // chi planes per slab
+            const size_t nchi = cps * ns;
+            const cplx* chi0 = chi + (size_t)s0 * cps * h->M;
+            for (size_t q0 = 0; q0 < nchi; q0 += (size_t)h->nbz) {
+                const int nb = (int)((nchi - q0 < (size_t)h->nbz) ? nchi - q0 : (size_t)h->nbz);
+                GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(chi0 + q0 * h->M, s.Z, h->twx, h->nky0, nb, 0, h->kxmin, h->kymin)));
+                GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
+                launches += 2;
+            }
+            const size_t goff = (size_t)s0 * h->nz * h->nv * h->M;
+            long long T = (long long)ns * h->nz * h->nv;
+            int grid = (T < h->fused_grid) ? (int)T : h->fused_grid;
+            GNL_LAUNCH(prof, K_FUSED, (h->fk.fn<<<grid, h->fk.nt, h->fk.smem, st>>>(g + goff, rhs + goff, s.R, h->twx, h->twy, h->nz, h->nv, ns, h->chi_has_v, h->kxmin, h->kymin, coef)));
+            launches += 1;
+        }
+        if (!cuda_ok(cudaGetLastError(), "kernel launch")) return -1;
+        return launches;
+    }
+    for (int sl = 0; sl < nslab; ++sl) {
+        for (int z0 = 0; z0 < h->nz; z0 += h->nzb) {
+            const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
+            const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * sl) * h->M;
+            const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * sl) * h->M;
+            int n = enqueue_chunk(h, s, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, st, prof);
+            if (n < 0) return -1;
+            launches += n;
+        }
+    }
+    return launches;
+}
+
 int chunks_per_slab(const gene_nl_plan* h) { return (h->nz + h->nzb - 1) / h->nzb; }
 
 int launches_per_chunk(const gene_nl_plan* h)
@@ -274,7 +358,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     h->M = (size_t)nx0 * nky0;
     h->planes = (long long)nz * nv * nw * nspec;
     h->device = dev;
-    if (!find_x(h->Nx, &h->xk) || !find_y(h->Ny, &h->yk)) {
+    if (!find_x(h->Nx, &h->xk) || !find_y(h->Ny, h->Nx, &h->yk)) {
         char buf[160];
         snprintf(buf, sizeof buf, "gene_nl_create: unsupported padded grid %dx%d (Nx in {24,48,96,144,192,384,768}, Ny in {24,48,96,144,192,384})", h->Nx, h->Ny);
         set_err(buf);
@@ -306,10 +390,33 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     h->pbytes = ppp * nb;
     h->rbytes = rpp * (h->chi_has_v ? nb : (size_t)nzb);
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
+    {
+        const char* e = getenv("GENE_NL_NO_FUSED");  // development knob: force the batched kernels
+        h->fused = !(e && atoi(e)) && find_fused(h->Nx, h->Ny, &h->fk);
+    }
+    if (h->fused) {
+        int sms = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        h->fused_grid = sms > 0 ? sms : 148;
+        const size_t cps = (size_t)nz * (h->chi_has_v ? nv : 1);      // chi planes per slab
+        const size_t rcap = (size_t)2 << 30;                          // real-space chi kept per launch
+        size_t nss = rcap / (cps * rpp);
+        if (nss < 1) nss = 1;
+        if (nss > (size_t)nw * nspec) nss = (size_t)nw * nspec;
+        h->nss = (int)nss;
+        size_t nbz = ((size_t)64 << 20) / zpp;
+        if (nbz < 1) nbz = 1;
+        if (nbz > cps * nss) nbz = cps * nss;
+        h->nbz = (long long)nbz;
+        h->zbytes = zpp * nbz;
+        h->pbytes = 256;
+        h->rbytes = rpp * cps * nss;
+    }
 
     bool ok = upload_twiddles(h->Nx, &h->twx) && upload_twiddles(h->Ny, &h->twy) && alloc_scratch(h, &h->scr) &&
               set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
-              set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem");
+              set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
+              (!h->fused || set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"));
     if (!ok) {
         std::string keep = g_err;
         gene_nl_destroy(h);
@@ -357,16 +464,8 @@ static int compute_impl(gene_nl_plan* h, const void* chi_, const void* g_, void*
     const cplx* g = (const cplx*)g_;
     cplx* rhs = (cplx*)rhs_;
     cudaStream_t st = (cudaStream_t)stream;
-    for (int ws = 0; ws < h->nw * h->nspec; ++ws) {
-        for (int z0 = 0; z0 < h->nz; z0 += h->nzb) {
-            const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
-            const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * ws) * h->M;
-            const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * ws) * h->M;
-            if (prof) prof->st = st;
-            if (enqueue_chunk(h, h->scr, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, st, prof) < 0)
-                return GENE_NL_ECUDA;
-        }
-    }
+    if (prof) prof->st = st;
+    if (enqueue_slabs(h, h->scr, chi, g, rhs, h->nw * h->nspec, scale, st, prof) < 0) return GENE_NL_ECUDA;
     return GENE_NL_OK;
 }
 
@@ -376,7 +475,7 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, 
 }
 
 int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale, void* stream,
-                             double* ms4, int* launches4)
+                             double* ms4, int* launches4)  /* arrays of GENE_NL_KERNEL_CLASSES entries */
 {
     if (!ms4 || !launches4) { set_err("NULL output pointer"); return GENE_NL_EINVAL; }
     Profiler prof;
@@ -404,45 +503,32 @@ int gene_nl_compute_host(gene_nl_plan* h, const void* chi_, const void* g_, void
     const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
     int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
     if (rc) return rc;
-    const size_t pb = sizeof(cplx) * h->M;  // plane bytes
-    const size_t chunk_planes = (size_t)h->nzb * h->nv;
+    // one chunk = one (w,s) slab: nz*nv contiguous planes of g and rhs, nz (or nz*nv) planes of chi
+    const size_t slab_g = sizeof(cplx) * h->M * (size_t)h->nz * h->nv;
+    const size_t slab_c = h->chi_has_v ? slab_g : slab_g / h->nv;
     if (h->stages.empty()) {
         const int nstage = 3;
         h->stages.resize(nstage);
         for (auto& s : h->stages) {
             bool ok = cuda_ok(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate") &&
-                      cuda_ok(cudaMalloc(&s.g, chunk_planes * pb), "cudaMalloc(stage g)") &&
-                      cuda_ok(cudaMalloc(&s.rhs, chunk_planes * pb), "cudaMalloc(stage rhs)") &&
-                      cuda_ok(cudaMalloc(&s.chi, (h->chi_has_v ? chunk_planes : (size_t)h->nzb) * pb), "cudaMalloc(stage chi)") &&
-                      alloc_scratch(h, &s.scr);
+                      cuda_ok(cudaMalloc(&s.g, slab_g), "cudaMalloc(stage g)") &&
+                      cuda_ok(cudaMalloc(&s.rhs, slab_g), "cudaMalloc(stage rhs)") &&
+                      cuda_ok(cudaMalloc(&s.chi, slab_c), "cudaMalloc(stage chi)") && alloc_scratch(h, &s.scr);
             if (!ok) return GENE_NL_ENOMEM;
         }
     }
     const char* chi = (const char*)chi_;
     const char* g = (const char*)g_;
     char* rhs = (char*)rhs_;
-    int k = 0;
     for (int ws = 0; ws < h->nw * h->nspec; ++ws) {
-        for (int z0 = 0; z0 < h->nz; z0 += h->nzb, ++k) {
-            HostStage& s = h->stages[k % h->stages.size()];
-            const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
-            const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * ws) * pb;
-            const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * ws) * pb;
-            // rows = v, width = nzc contiguous planes; host pitch nz planes, staging pitch nzc planes
-            const size_t width = (size_t)nzc * pb, hpitch = (size_t)h->nz * pb;
-            bool ok = cuda_ok(cudaMemcpy2DAsync(s.g, width, g + goff, hpitch, width, h->nv, cudaMemcpyHostToDevice, s.stream), "H2D g") &&
-                      cuda_ok(cudaMemcpy2DAsync(s.rhs, width, rhs + goff, hpitch, width, h->nv, cudaMemcpyHostToDevice, s.stream), "H2D rhs");
-            if (ok) {
-                if (h->chi_has_v)
-                    ok = cuda_ok(cudaMemcpy2DAsync(s.chi, width, chi + coff, hpitch, width, h->nv, cudaMemcpyHostToDevice, s.stream), "H2D chi");
-                else
-                    ok = cuda_ok(cudaMemcpyAsync(s.chi, chi + coff, width, cudaMemcpyHostToDevice, s.stream), "H2D chi");
-            }
-            if (!ok) return GENE_NL_ECUDA;
-            if (enqueue_chunk(h, s.scr, s.chi, nzc, s.g, s.rhs, nzc, nzc, scale, s.stream) < 0) return GENE_NL_ECUDA;
-            if (!cuda_ok(cudaMemcpy2DAsync(rhs + goff, hpitch, s.rhs, width, width, h->nv, cudaMemcpyDeviceToHost, s.stream), "D2H rhs"))
-                return GENE_NL_ECUDA;
-        }
+        HostStage& s = h->stages[ws % h->stages.size()];
+        bool ok = cuda_ok(cudaMemcpyAsync(s.g, g + ws * slab_g, slab_g, cudaMemcpyHostToDevice, s.stream), "H2D g") &&
+                  cuda_ok(cudaMemcpyAsync(s.rhs, rhs + ws * slab_g, slab_g, cudaMemcpyHostToDevice, s.stream), "H2D rhs") &&
+                  cuda_ok(cudaMemcpyAsync(s.chi, chi + ws * slab_c, slab_c, cudaMemcpyHostToDevice, s.stream), "H2D chi");
+        if (!ok) return GENE_NL_ECUDA;
+        if (enqueue_slabs(h, s.scr, s.chi, s.g, s.rhs, 1, scale, s.stream) < 0) return GENE_NL_ECUDA;
+        if (!cuda_ok(cudaMemcpyAsync(rhs + ws * slab_g, s.rhs, slab_g, cudaMemcpyDeviceToHost, s.stream), "D2H rhs"))
+            return GENE_NL_ECUDA;
     }
     for (auto& s : h->stages)
         if (!cuda_ok(cudaStreamSynchronize(s.stream), "cudaStreamSynchronize")) return GENE_NL_ECUDA;
@@ -458,7 +544,17 @@ size_t gene_nl_workspace_bytes(const gene_nl_plan* h)
 int gene_nl_launches_per_compute(const gene_nl_plan* h)
 {
     if (!h) return 0;
-    return h->nw * h->nspec * chunks_per_slab(h) * launches_per_chunk(h);
+    const int nslab = h->nw * h->nspec;
+    if (h->fused) {
+        int n = 0;
+        const size_t cps = (size_t)h->nz * (h->chi_has_v ? h->nv : 1);
+        for (int s0 = 0; s0 < nslab; s0 += h->nss) {
+            const int ns = (nslab - s0 < h->nss) ? nslab - s0 : h->nss;
+            n += 2 * (int)((cps * ns + (size_t)h->nbz - 1) / (size_t)h->nbz) + 1;
+        }
+        return n;
+    }
+    return nslab * chunks_per_slab(h) * launches_per_chunk(h);
 }
 
 double gene_nl_query(const gene_nl_plan* h, int what)
@@ -470,8 +566,10 @@ double gene_nl_query(const gene_nl_plan* h, int what)
     case 0: return (double)h->planes;
     case 1: return Nx;
     case 2: return Ny;
-    case 3: return (double)h->nzb * h->nvb;
-    case 4: return (double)h->nw * h->nspec * chunks_per_slab(h) * ((h->nv + h->nvb - 1) / h->nvb);
+    case 3: return h->fused ? (double)h->nss * h->nz * h->nv : (double)h->nzb * h->nvb;
+    case 4: return h->fused ? (double)((h->nw * h->nspec + h->nss - 1) / h->nss)
+                            : (double)h->nw * h->nspec * chunks_per_slab(h) * ((h->nv + h->nvb - 1) / h->nvb);
+    case 7: return h->fused ? 1.0 : 0.0;
     case 5: return 16.0 * M * (3.0 + c);
     case 6: {
         const double t2d = h->nky0 * 5.0 * Nx * std::log2(Nx) + Nx * 2.5 * Ny * std::log2(Ny);

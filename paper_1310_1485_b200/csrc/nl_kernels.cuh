@@ -29,12 +29,20 @@ __host__ __device__ constexpr int odd_up(int v) { return v | 1; }
 template <int A, int B>
 struct Tile {
     static constexpr int BP = odd_up(B);
-    static constexpr int STRIDE = odd_up(A * BP);
+    static constexpr int STRIDE = odd_up(A * BP);  // x kernels: lanes run over columns (stride must be odd)
+    static constexpr int FLAT = A * BP;            // y kernels: lanes run over (row, k1) as one flat index
 };
 
-__device__ __forceinline__ void load_twiddles(cplx* tw_s, const cplx* __restrict__ tw_g, int n)
+// Twiddle table of one length N = A*B in shared memory, laid out [k1][n2] with row stride BP (odd):
+// T[k1*BP + n2] = W_N^{n2 k1}.  Conflict-free both for lanes over n2 and for lanes over k1.
+template <int A, int B>
+__device__ __forceinline__ void load_twiddles_ab(cplx* tw_s, const cplx* __restrict__ tw_g)
 {
-    for (int t = threadIdx.x; t < n; t += blockDim.x) tw_s[t] = tw_g[t];
+    constexpr int BP = Tile<A, B>::BP;
+    for (int t = threadIdx.x; t < A * B; t += blockDim.x) {
+        const int k1 = t / B, n2 = t % B;
+        tw_s[k1 * BP + n2] = tw_g[k1 * n2];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -51,7 +59,7 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
     constexpr int BP = Tile<A, B>::BP, CS = Tile<A, B>::STRIDE;
     extern __shared__ cplx smem[];
     cplx* tw = smem;
-    cplx* E = smem + NX;
+    cplx* E = smem + A * BP;
 
     const int ntile = nky0 / CK;
     const int bl = blockIdx.x / ntile;
@@ -60,7 +68,7 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
     const cplx* F = src + ((size_t)(bl % nzb) + (size_t)vstride * (bl / nzb)) * ((size_t)NX0 * nky0);
     cplx* Zb = Z + (size_t)bl * NX * W2;
 
-    load_twiddles(tw, tw_g, NX);
+    load_twiddles_ab<A, B>(tw, tw_g);
     __syncthreads();
 
     // stage 1: pruned radix-A over n1 for fixed n2 (n = n2 + B*n1), then twiddle W_NX^{n2 k1}
@@ -102,7 +110,7 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
         cplx* Ec = E + c2 * CS + n2;
 #pragma unroll
         for (int k1 = 0; k1 < A; ++k1) {
-            cplx w = tw[n2 * k1];
+            cplx w = tw[k1 * BP + n2];
             Ec[k1 * BP] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
         }
     }
@@ -146,7 +154,7 @@ __device__ __forceinline__ void y_stage1(const cplx* __restrict__ Zr, const cplx
     dft_pruned_in<A, +1>(lo, hi, out);
 #pragma unroll
     for (int k1 = 0; k1 < A; ++k1) {
-        cplx w = tw[n2 * k1];
+        cplx w = tw[k1 * BP + n2];
         Er[k1 * BP + n2] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
     }
 }
@@ -159,14 +167,14 @@ __global__ void __launch_bounds__(NT)
 k_yreal(const cplx* __restrict__ Z, cplx* __restrict__ R, const cplx* __restrict__ tw_g, int Nx)
 {
     constexpr int W2 = 2 * (NY / 3);
-    constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::STRIDE;
+    constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
     extern __shared__ cplx smem[];
     cplx* tw = smem;
-    cplx* E = smem + NY;
+    cplx* E = smem + RS;
     const int ntile = Nx / RT;
     const int ql = blockIdx.x / ntile;
     const int m0 = (blockIdx.x % ntile) * RT;
-    load_twiddles(tw, tw_g, NY);
+    load_twiddles_ab<A, B>(tw, tw_g);
     __syncthreads();
     for (int item = threadIdx.x; item < RT * B; item += NT) {
         const int n2 = item % B, r = item / B;
@@ -196,16 +204,16 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
            const cplx* __restrict__ tw_g, int Nx, int nzb, int chi_per_plane)
 {
     constexpr int A1 = A / 3, NKY0 = NY / 3, W2 = 2 * NKY0;
-    constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::STRIDE;
+    constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
     extern __shared__ cplx smem[];
     cplx* tw = smem;
-    cplx* E = smem + NY;
+    cplx* E = smem + RS;
     const int half = Nx / 2;
     const int ntile = half / RP;
     const int bl = blockIdx.x / ntile;
     const int m0 = (blockIdx.x % ntile) * RP;
     const int ql = chi_per_plane ? bl : bl % nzb;
-    load_twiddles(tw, tw_g, NY);
+    load_twiddles_ab<A, B>(tw, tw_g);
     __syncthreads();
 
     // Y1: pruned radix-A + twiddle for the 2*RP rows of the tile
@@ -241,7 +249,7 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
         cplx* Er = E + r * RS + k1 * BP;
 #pragma unroll
         for (int k2 = 0; k2 < B; ++k2) {
-            cplx t = tw[k1 * k2];
+            cplx t = tw[k1 * BP + k2];
             Er[k2] = (k2 == 0) ? w[0] : cmul(w[k2], t.x, -t.y);
         }
     }
@@ -278,14 +286,14 @@ k_xfwd(const cplx* __restrict__ P, cplx* __restrict__ rhs, const cplx* __restric
     constexpr int BP = Tile<A, B>::BP, CS = Tile<A, B>::STRIDE;
     extern __shared__ cplx smem[];
     cplx* tw = smem;
-    cplx* E = smem + NX;
+    cplx* E = smem + A * BP;
     const int ntile = nky0 / CK;
     const int bl = blockIdx.x / ntile;
     const int ky0 = (blockIdx.x % ntile) * CK;
     const int W2 = 2 * nky0;
     const cplx* Pb = P + (size_t)bl * HALF * W2;
     cplx* Rb = rhs + ((size_t)(bl % nzb) + (size_t)vstride * (bl / nzb)) * ((size_t)NX0 * nky0);
-    load_twiddles(tw, tw_g, NX);
+    load_twiddles_ab<A, B>(tw, tw_g);
     __syncthreads();
 
     // stage 1: unpack the row pair, radix-B over n2 for fixed n1 (m = n1 + A*n2), twiddle W^{-n1 k2}
@@ -305,7 +313,7 @@ k_xfwd(const cplx* __restrict__ P, cplx* __restrict__ rhs, const cplx* __restric
         cplx* Ec = E + col * CS + n1 * BP;
 #pragma unroll
         for (int k2 = 0; k2 < B; ++k2) {
-            cplx t = tw[n1 * k2];
+            cplx t = tw[n1 * BP + k2];
             Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], t.x, -t.y);
         }
     }
