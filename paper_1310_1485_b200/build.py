@@ -9,7 +9,6 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgene_nl.so")
 SOURCES = ["gene_nl.cu", "probe.cu"]
-HEADERS = ["nl_kernels.cuh", "dft_regs.cuh", "twiddle_consts.cuh", os.path.join("..", "..", "include", "gene_nl.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]
 
@@ -25,7 +24,8 @@ def is_stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS]
+    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
+    deps.append(os.path.join(HERE, "..", "include", "gene_nl.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -37,13 +37,26 @@ struct Fused {
     static_assert(AX % 3 == 0 && AY % 3 == 0, "3/2 rule");
     static_assert(AY <= 16, "two pairs per Y2 pass need AY <= 16");
 
+    // offset of row m of Z (rows m and m + NPAIR share one pair storage)
     __device__ static __forceinline__ int zrow(int m) { return (m % NPAIR) * PS + (m / NPAIR) * W2; }
+    // offset of the 8-row group that holds the x tile slots (k1, *): rows 8 k1 .. 8 k1 + 7
+    __device__ static __forceinline__ int tile_group(int k1)
+    {
+        if constexpr (NPAIR % 8 == 0) {
+            const int half = (8 * k1 >= NPAIR) ? 1 : 0;
+            return (8 * k1 - NPAIR * half) * PS + half * W2;
+        } else {
+            return -1;  // rows of a group may straddle the two halves: use zrow per row
+        }
+    }
+    __device__ static __forceinline__ int tile_slot(int k1, int s)  // s = (n2 + k1) & 7
+    {
+        if constexpr (NPAIR % 8 == 0)
+            return tile_group(k1) + s * PS;
+        else
+            return zrow(8 * k1 + s);
+    }
 };
-
-__device__ __forceinline__ cplx ldg_nc(const cplx* p)
-{
-    return __ldg(p);
-}
 
 // An opaque copy of a lane-constant value: keeps the compiler from hoisting per-lane address and
 // wavenumber arithmetic out of the plane loop (where it would sit in registers for the whole kernel).
@@ -56,6 +69,65 @@ __device__ __forceinline__ int opaque(int v)
 __device__ __forceinline__ void prefetch_l2(const void* p)
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
+// (i kx + kys) * f
+__device__ __forceinline__ cplx deriv_mul(cplx f, double kx, double kys)
+{
+    return cmake(fma(kys, f.x, -kx * f.y), fma(kx, f.x, kys * f.y));
+}
+
+// X-inv stage 1 for one lane: column (kyi, sg), position n2.  KY0: the pass that contains ky = 0
+// (Hermitian part of the ky = 0 column, reading R7; and the all-zero column cc = NKY0).
+template <class C, int AX, bool KY0>
+__device__ __forceinline__ void xinv_stage1(cplx* Z, const cplx* twx, const cplx* __restrict__ F, int u, int lane,
+                                            double kxmin, double kymin)
+{
+    constexpr int AX1 = AX / 3, M = C::M, NX0 = C::NX0, W2 = C::W2, NKY0 = C::NKY0, PS = C::PS;
+    const int n2 = lane & 7, sg = (lane >> 3) & 1, kyi = 2 * u + (lane >> 4);
+    const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
+    const cplx* Fc = F + (size_t)kyi * NX0 + n2;
+    const double ky = kymin * (double)kyi;
+    const double kys = sg ? ky : -ky;  // (i kx - ky) F for +ky, (i kx + ky) F for -ky
+    const double dn2 = (double)n2;
+    cplx lo[AX1], hi[AX1];
+#pragma unroll
+    for (int a = 0; a < AX1; ++a) {
+        cplx f0 = Fc[8 * a], f1 = Fc[8 * a + M];
+        if constexpr (KY0) {
+            if (kyi == 0) {
+                const int i0 = n2 + 8 * a, i1 = i0 + M;
+                cplx m0 = F[(NX0 - i0) % NX0], m1 = F[NX0 - i1];
+                f0 = cmake(0.5 * (f0.x + m0.x), 0.5 * (f0.y - m0.y));
+                f1 = cmake(0.5 * (f1.x + m1.x), 0.5 * (f1.y - m1.y));
+            }
+        }
+        const double kx0 = kxmin * (dn2 + (double)(8 * a));             // i = n2 + 8a        (kx >= 0)
+        const double kx1 = kxmin * (dn2 + (double)(8 * a + M - NX0));   // i = n2 + 8a + M    (kx < 0)
+        lo[a] = deriv_mul(f0, kx0, kys);
+        hi[a] = deriv_mul(f1, kx1, kys);
+        if (a == 0 && n2 == 0) hi[0] = cmake(0.0, 0.0);  // i = M: the Nyquist row is ignored (R6)
+    }
+    cplx out[AX];
+    dft_pruned_in<AX, +1>(lo, hi, out);
+    if constexpr (KY0) {
+        if (sg && kyi == 0) {  // there is no -0 column: slot cc = NKY0 holds zeros
+#pragma unroll
+            for (int k1 = 0; k1 < AX; ++k1) out[k1] = cmake(0.0, 0.0);
+        }
+    }
+    int soff[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) soff[r] = ((n2 + r) & 7) * PS + cc;
+#pragma unroll
+    for (int k1 = 0; k1 < AX; ++k1) {
+        const cplx w = twx[k1 * 9 + n2];
+        const cplx val = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
+        if constexpr (C::NPAIR % 8 == 0)
+            Z[C::tile_group(k1) + soff[k1 & 7]] = val;
+        else
+            Z[C::zrow(8 * k1 + ((n2 + k1) & 7)) + cc] = val;
+    }
 }
 
 template <int AX, int AY, int NW>
@@ -111,49 +183,12 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         // ---------------- X-inv: 2 stored columns x {+ky, -ky} per warp pass --------------------
         for (int u = warp; u < NKY0 / 2; u += NW) {
             const int lane = opaque(lane0);
-            {
-                const int n2 = lane & 7, sg = (lane >> 3) & 1, kyi = 2 * u + (lane >> 4);
-                const bool zero = sg && kyi == 0;  // there is no -0 column: slot cc = NKY0 holds zeros
-                const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
-                const cplx* Fc = F + (size_t)kyi * NX0;
-                const double ky = kymin * (double)kyi;
-                const double kys = sg ? ky : -ky;
-                cplx lo[AX1], hi[AX1];
-#pragma unroll
-                for (int a = 0; a < AX1; ++a) {
-                    {
-                        const int i = n2 + 8 * a;
-                        const double kx = kxmin * (double)i;
-                        cplx f = Fc[i];
-                        if (kyi == 0) {
-                            cplx fm = Fc[(NX0 - i) % NX0];
-                            f = cmake(0.5 * (f.x + fm.x), 0.5 * (f.y - fm.y));
-                        }
-                        lo[a] = cmake(fma(kys, f.x, -kx * f.y), fma(kx, f.x, kys * f.y));
-                    }
-                    {
-                        const int i = n2 + 8 * a + M;
-                        const double kx = kxmin * (double)(i - NX0);
-                        cplx f = Fc[i];
-                        if (kyi == 0) {
-                            cplx fm = Fc[NX0 - i];
-                            f = cmake(0.5 * (f.x + fm.x), 0.5 * (f.y - fm.y));
-                        }
-                        cplx val = cmake(fma(kys, f.x, -kx * f.y), fma(kx, f.x, kys * f.y));
-                        hi[a] = (i == M) ? cmake(0.0, 0.0) : val;
-                    }
-                }
-                cplx out[AX];
-                dft_pruned_in<AX, +1>(lo, hi, out);
-#pragma unroll
-                for (int k1 = 0; k1 < AX; ++k1) {
-                    const int row = 8 * k1 + ((n2 + k1) & 7);
-                    cplx w = twx[k1 * 9 + n2];
-                    cplx val = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
-                    Z[C::zrow(row) + cc] = zero ? cmake(0.0, 0.0) : val;
-                }
-            }
+            if (u == 0)
+                xinv_stage1<C, AX, true>(Z, twx, F, u, lane, kxmin, kymin);
+            else
+                xinv_stage1<C, AX, false>(Z, twx, F, u, lane, kxmin, kymin);
             __syncwarp(FULL);
+            // stage 2: every lane first reads ALL its tile slots (the outputs overwrite the same column)
             cplx vv[NJ][8];
 #pragma unroll
             for (int j = 0; j < NJ; ++j) {
@@ -162,8 +197,14 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     const int cidx = item / AX, k1 = item % AX;
                     const int sg = cidx & 1, kyi = 2 * u + (cidx >> 1);
                     const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
+                    if constexpr (NPAIR % 8 == 0) {
+                        const cplx* Zt = Z + C::tile_group(k1) + cc;
 #pragma unroll
-                    for (int n2 = 0; n2 < 8; ++n2) vv[j][n2] = Z[C::zrow(8 * k1 + ((n2 + k1) & 7)) + cc];
+                        for (int n2 = 0; n2 < 8; ++n2) vv[j][n2] = Zt[((n2 + k1) & 7) * PS];
+                    } else {
+#pragma unroll
+                        for (int n2 = 0; n2 < 8; ++n2) vv[j][n2] = Z[C::zrow(8 * k1 + ((n2 + k1) & 7)) + cc];
+                    }
                 }
             }
             __syncwarp(FULL);
@@ -175,9 +216,11 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     const int sg = cidx & 1, kyi = 2 * u + (cidx >> 1);
                     const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
                     Dft<8, +1>::run(vv[j]);
+                    cplx* Zo = Z + k1 * PS + cc;  // row k1 + AX*k2: first half for k2 < 4 (k1 < AX, NPAIR = 4 AX)
+                    const double sgn = sg ? -1.0 : 1.0;
 #pragma unroll
                     for (int k2 = 0; k2 < 8; ++k2)
-                        Z[C::zrow(k1 + AX * k2) + cc] = sg ? cconj(vv[j][k2]) : vv[j][k2];
+                        Zo[(k2 < 4) ? AX * k2 * PS : AX * (k2 - 4) * PS + W2] = cmake(vv[j][k2].x, sgn * vv[j][k2].y);
                 }
             }
         }
@@ -196,53 +239,52 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 for (int h = 0; h < 2; ++h) {
                     const cplx* Rr = Rc + (size_t)(pair2 + h * NPAIR) * NY + k1y;
 #pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc(Rr + AY * k2);
+                    for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = __ldg(Rr + AY * k2);
                 }
             }
             {  // Y1: pruned radix-AY + twiddle, 4 rows x 8 lanes
                 const int ridx = lane >> 3, n2 = lane & 7;
                 const int pair1 = 2 * u + (ridx >> 1), h1 = ridx & 1;
-                const cplx* Zr = Z + pair1 * PS + h1 * W2;
-                cplx lo[AY1], hi[AY1];
+                const cplx* Zr = Z + pair1 * PS + h1 * W2 + n2;
+                cplx lo[AY1], hi[AY1], tw[AY];
 #pragma unroll
                 for (int a = 0; a < AY1; ++a) {
-                    lo[a] = Zr[n2 + 8 * a];
-                    hi[a] = Zr[n2 + 8 * a + NKY0];
+                    lo[a] = Zr[8 * a];
+                    hi[a] = Zr[8 * a + NKY0];
                 }
+#pragma unroll
+                for (int k1 = 1; k1 < AY; ++k1) tw[k1] = twy[k1 * 9 + n2];
                 cplx out[AY];
                 dft_pruned_in<AY, +1>(lo, hi, out);
                 __syncwarp(FULL);  // every lane has read its row before the tiles overwrite the pair storage
-                cplx* tile = h1 ? ST + (warp * 2 + (ridx >> 1)) * FY : Z + pair1 * PS;
+                cplx* tile = (h1 ? ST + (warp * 2 + (ridx >> 1)) * FY : Z + pair1 * PS) + n2;
+                tile[0] = out[0];
 #pragma unroll
-                for (int k1 = 0; k1 < AY; ++k1) {
-                    cplx w = twy[k1 * 9 + n2];
-                    tile[k1 * 9 + n2] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
-                }
+                for (int k1 = 1; k1 < AY; ++k1) tile[k1 * 9] = cmul(out[k1], tw[k1].x, tw[k1].y);
             }
             __syncwarp(FULL);
             if (act2) {  // Y2: to real space (both rows), bracket, back; result replaces tile 0 in place
+                cplx* tile0 = Z + pair2 * PS + k1y * 9;
+                const cplx* tile1 = ST + (warp * 2 + pidx2) * FY + k1y * 9;
+                cplx v0[8], v1[8], tq[8];
+#pragma unroll
+                for (int n2 = 0; n2 < 8; ++n2) v0[n2] = tile0[n2];
+#pragma unroll
+                for (int n2 = 0; n2 < 8; ++n2) v1[n2] = tile1[n2];
+#pragma unroll
+                for (int k2 = 1; k2 < 8; ++k2) tq[k2] = twy[k1y * 9 + k2];
+                Dft<8, +1>::run(v0);
+                Dft<8, +1>::run(v1);
                 cplx w[8];
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const cplx* tile = h ? ST + (warp * 2 + pidx2) * FY : Z + pair2 * PS;
-                    cplx vr[8];
-#pragma unroll
-                    for (int n2 = 0; n2 < 8; ++n2) vr[n2] = tile[k1y * 9 + n2];
-                    Dft<8, +1>::run(vr);
-#pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) {
-                        const cplx c = chv[h][k2];
-                        const double nl = fma(c.x, vr[k2].y, -c.y * vr[k2].x);
-                        if (h == 0) w[k2].x = nl; else w[k2].y = nl;
-                    }
+                for (int k2 = 0; k2 < 8; ++k2) {  // dx chi * dy g - dy chi * dx g for rows m and m + NX/2
+                    w[k2].x = fma(chv[0][k2].x, v0[k2].y, -chv[0][k2].y * v0[k2].x);
+                    w[k2].y = fma(chv[1][k2].x, v1[k2].y, -chv[1][k2].y * v1[k2].x);
                 }
                 Dft<8, -1>::run(w);
-                cplx* tile0 = Z + pair2 * PS + k1y * 9;
+                tile0[0] = w[0];
 #pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) {
-                    cplx tq = twy[k1y * 9 + k2];
-                    tile0[k2] = (k2 == 0) ? w[0] : cmul(w[k2], tq.x, -tq.y);
-                }
+                for (int k2 = 1; k2 < 8; ++k2) tile0[k2] = cmul(w[k2], tq[k2].x, -tq[k2].y);
             }
             __syncwarp(FULL);
             {  // Y3: pruned-output radix-AY; P[pair][cc] overwrites tile 0 after everyone has read it
@@ -278,13 +320,13 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 if (item < 4 * AX) {
                     const int col = item / AX, n1 = item % AX;
                     const int kyi = 4 * u + col;
-                    const int ccp = kyi, ccm = kyi ? W2 - kyi : 0;
+                    const cplx* Pp = Z + n1 * PS + kyi;
+                    const cplx* Pm = Z + n1 * PS + (kyi ? W2 - kyi : 0);
 #pragma unroll
-                    for (int n2 = 0; n2 < 4; ++n2) {
-                        const cplx* Pr = Z + (n1 + AX * n2) * PS;
-                        const cplx pp = Pr[ccp], pm = Pr[ccm];
-                        xx[j][n2] = cmake(pp.x + pm.x, pp.y - pm.y);
-                        xx[j][n2 + 4] = cmake(pp.y + pm.y, pm.x - pp.x);
+                    for (int n2 = 0; n2 < 4; ++n2) {  // rows m = n1 + AX n2 and m + NX/2 of pair n1 + AX n2
+                        const cplx pp = Pp[AX * n2 * PS], pm = Pm[AX * n2 * PS];
+                        xx[j][n2] = cmake(pp.x + pm.x, pp.y - pm.y);      // 2 N^_m  = P+ + conj P-
+                        xx[j][n2 + 4] = cmake(pp.y + pm.y, pm.x - pp.x);  // 2 N^_m' = -i (P+ - conj P-)
                     }
                 }
             }
@@ -296,13 +338,25 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     const int col = item / AX, n1 = item % AX;
                     const int kyi = 4 * u + col;
                     const int s0 = kyi, s1 = kyi ? W2 - kyi : NKY0;
-                    Dft<8, -1>::run(xx[j]);
+                    cplx tq[8];
 #pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) {
-                        const int e = 8 * n1 + ((k2 + n1) & 7);
-                        cplx tq = twx[n1 * 9 + k2];
-                        Z[(e % NPAIR) * PS + ((e / NPAIR) ? s1 : s0)] =
-                            (k2 == 0) ? xx[j][0] : cmul(xx[j][k2], tq.x, -tq.y);
+                    for (int k2 = 1; k2 < 8; ++k2) tq[k2] = twx[n1 * 9 + k2];
+                    Dft<8, -1>::run(xx[j]);
+                    if constexpr (NPAIR % 8 == 0) {
+                        // tile slot (n1,k2) -> row 8 n1 + ((k2+n1)&7); second-half rows use slot s1 of their pair
+                        const int half = (8 * n1 >= NPAIR) ? 1 : 0;
+                        cplx* Zt = Z + (8 * n1 - NPAIR * half) * PS + (half ? s1 : s0);
+                        Zt[(n1 & 7) * PS] = xx[j][0];
+#pragma unroll
+                        for (int k2 = 1; k2 < 8; ++k2)
+                            Zt[((k2 + n1) & 7) * PS] = cmul(xx[j][k2], tq[k2].x, -tq[k2].y);
+                    } else {
+#pragma unroll
+                        for (int k2 = 0; k2 < 8; ++k2) {
+                            const int e = 8 * n1 + ((k2 + n1) & 7);
+                            Z[(e % NPAIR) * PS + ((e / NPAIR) ? s1 : s0)] =
+                                (k2 == 0) ? xx[j][0] : cmul(xx[j][k2], tq[k2].x, -tq[k2].y);
+                        }
                     }
                 }
             }
@@ -311,27 +365,34 @@ k_plane_fused(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 const int col = lane >> 3, k2 = lane & 7;
                 const int kyi = 4 * u + col;
                 const int s0 = kyi, s1 = kyi ? W2 - kyi : NKY0;
-                cplx* Rcol = Rb + (size_t)kyi * NX0;
-                cplx r0[AX1], r1[AX1];
-#pragma unroll
-                for (int c = 0; c < AX1; ++c) {  // rhs requested before the butterfly
-                    r0[c] = Rcol[k2 + 8 * c];
-                    r1[c] = Rcol[k2 + 8 * c + M];
-                }
                 cplx in[AX];
+                if constexpr (NPAIR % 8 == 0) {
+                    int soff[8];
 #pragma unroll
-                for (int n1 = 0; n1 < AX; ++n1) {
-                    const int e = 8 * n1 + ((k2 + n1) & 7);
-                    in[n1] = Z[(e % NPAIR) * PS + ((e / NPAIR) ? s1 : s0)];
+                    for (int r = 0; r < 8; ++r) soff[r] = ((k2 + r) & 7) * PS;
+#pragma unroll
+                    for (int n1 = 0; n1 < AX; ++n1) {
+                        const int half = (8 * n1 >= NPAIR) ? 1 : 0;
+                        in[n1] = Z[(8 * n1 - NPAIR * half) * PS + soff[n1 & 7] + (half ? s1 : s0)];
+                    }
+                } else {
+#pragma unroll
+                    for (int n1 = 0; n1 < AX; ++n1) {
+                        const int e = 8 * n1 + ((k2 + n1) & 7);
+                        in[n1] = Z[(e % NPAIR) * PS + ((e / NPAIR) ? s1 : s0)];
+                    }
                 }
                 cplx lo[AX1], hi[AX1];
                 dft_pruned_out<AX, -1>(in, lo, hi);
+                cplx* Rcol = Rb + (size_t)kyi * NX0 + k2;
 #pragma unroll
-                for (int c = 0; c < AX1; ++c) {
-                    const int i = k2 + 8 * c;
-                    Rcol[i] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));
-                    if (i != 0)  // i + M == M is the Nyquist row: untouched
-                        Rcol[i + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
+                for (int c = 0; c < AX1; ++c) {  // delete the padded modes, prefactor, add to rhs
+                    const cplx r0 = Rcol[8 * c];
+                    Rcol[8 * c] = cmake(fma(coef, lo[c].x, r0.x), fma(coef, lo[c].y, r0.y));
+                    if (c != 0 || k2 != 0) {  // i = M is the Nyquist row: untouched (R6)
+                        const cplx r1 = Rcol[8 * c + M];
+                        Rcol[8 * c + M] = cmake(fma(coef, hi[c].x, r1.x), fma(coef, hi[c].y, r1.y));
+                    }
                 }
             }
         }
