@@ -271,8 +271,10 @@ def main():
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
     traffic = None
     try:  # measured DRAM bytes per launch of the dominant kernel, from the committed ncu capture
-        t = json.load(open(os.path.join(ROOT, "profiles", "dram_traffic.json")))
-        traffic = t.get(wl.name, {}).get(dom)
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
+            if row["workload"] == wl.name and row["kernel"] == dom:
+                traffic = float(row["dram_bytes_per_launch"])
     except Exception:
         pass
     roofline = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
