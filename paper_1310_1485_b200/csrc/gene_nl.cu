@@ -17,6 +17,7 @@
 
 #include "../../include/gene_nl.h"
 #include "nl_fused.cuh"
+#include "nl_fused2.cuh"
 #include "nl_kernels.cuh"
 
 using gnl::cplx;
@@ -44,11 +45,37 @@ typedef void (*ybr_fn)(const cplx*, const cplx*, cplx*, const cplx*, int, int, i
 typedef void (*fused_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, int, double, double,
                          double);
 
+typedef void (*fused2_fn)(const cplx*, cplx*, const cplx*, const cplx*, int, int, int, int, double, double, double);
+
 struct FusedKernel {
     fused_fn fn = nullptr;
+    fused2_fn fn2 = nullptr;  // second-generation kernel (nl_fused2.cuh); used when available
     size_t smem = 0;
     int nt = 0;
 };
+
+template <int AX, int AY, int NW>
+FusedKernel make_fused2()
+{
+    FusedKernel k;
+    k.fn2 = gnl::k_plane_fused2<AX, AY, NW>;
+    k.smem = gnl::Fused2<AX, AY, NW>::SMEM_BYTES;
+    k.nt = NW * 32;
+    return k;
+}
+
+// nky0 a multiple of 32 (Ny = 96) and Nx = 8 AX <= 192: the warp-uniform-twiddle kernel
+bool find_fused2(int nx, int ny, FusedKernel* out)
+{
+    if (ny != 96) return false;
+    switch (nx) {
+    case 48: *out = make_fused2<6, 12, 8>(); break;
+    case 96: *out = make_fused2<12, 12, 8>(); break;
+    case 192: *out = make_fused2<24, 12, 8>(); break;
+    default: return false;
+    }
+    return out->smem <= 227 * 1024;
+}
 
 template <int AX, int AY, int NW>
 FusedKernel make_fused()
@@ -236,6 +263,23 @@ bool upload_twiddles(int n, cplx** out)
     return cuda_ok(cudaMemcpy(*out, t.data(), sizeof(cplx) * n, cudaMemcpyHostToDevice), "cudaMemcpy(twiddles)");
 }
 
+// W_N^j of every supported length into the __constant__ table read by the warp-uniform x stages
+bool upload_const_twiddles()
+{
+    static const int lens[] = {24, 48, 96, 144, 192, 384, 768};
+    std::vector<cplx> t(gnl::kCTwTotal);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int n : lens) {
+        const int off = gnl::ctw_offset(n);
+        for (int k = 0; k < n; ++k) {
+            long double ang = two_pi * (long double)k / (long double)n;
+            t[off + k].x = (double)cosl(ang);
+            t[off + k].y = (double)sinl(ang);
+        }
+    }
+    return cuda_ok(cudaMemcpyToSymbol(gnl::c_tw, t.data(), sizeof(cplx) * t.size()), "cudaMemcpyToSymbol(twiddles)");
+}
+
 template <class K>
 bool set_smem(K fn, size_t bytes, const char* name)
 {
@@ -306,7 +350,10 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const size_t goff = (size_t)s0 * h->nz * h->nv * h->M;
             long long T = (long long)ns * h->nz * h->nv;
             int grid = (T < h->fused_grid) ? (int)T : h->fused_grid;
-            GNL_LAUNCH(prof, K_FUSED, (h->fk.fn<<<grid, h->fk.nt, h->fk.smem, st>>>(g + goff, rhs + goff, s.R, h->twx, h->twy, h->nz, h->nv, ns, h->chi_has_v, h->kxmin, h->kymin, coef)));
+            if (h->fk.fn2)
+                GNL_LAUNCH(prof, K_FUSED, (h->fk.fn2<<<grid, h->fk.nt, h->fk.smem, st>>>(g + goff, rhs + goff, s.R, h->twy, h->nz, h->nv, ns, h->chi_has_v, h->kxmin, h->kymin, coef)));
+            else
+                GNL_LAUNCH(prof, K_FUSED, (h->fk.fn<<<grid, h->fk.nt, h->fk.smem, st>>>(g + goff, rhs + goff, s.R, h->twx, h->twy, h->nz, h->nv, ns, h->chi_has_v, h->kxmin, h->kymin, coef)));
             launches += 1;
         }
         if (!cuda_ok(cudaGetLastError(), "kernel launch")) return -1;
@@ -392,7 +439,9 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
     {
         const char* e = getenv("GENE_NL_NO_FUSED");  // development knob: force the batched kernels
-        h->fused = !(e && atoi(e)) && find_fused(h->Nx, h->Ny, &h->fk);
+        const char* e1 = getenv("GENE_NL_FUSED_V1");  // development knob: first-generation fused kernel
+        const bool want = !(e && atoi(e));
+        h->fused = want && ((!(e1 && atoi(e1)) && find_fused2(h->Nx, h->Ny, &h->fk)) || find_fused(h->Nx, h->Ny, &h->fk));
     }
     if (h->fused) {
         int sms = 0;
@@ -416,7 +465,9 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     bool ok = upload_twiddles(h->Nx, &h->twx) && upload_twiddles(h->Ny, &h->twy) && alloc_scratch(h, &h->scr) &&
               set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
               set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
-              (!h->fused || set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"));
+              (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
+                                       : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
+              upload_const_twiddles();
     if (!ok) {
         std::string keep = g_err;
         gene_nl_destroy(h);
