@@ -15,7 +15,10 @@
 //     7 complex values per lane per plane serve the two inverse rows and (conjugated) the forward row;
 //   * g is read once per column (the +ky and -ky syntheses share the loads), rhs values are requested
 //     before the last x stage so their latency hides behind it, Y3 runs on 4 pairs with all 32 lanes.
-// Phases of a plane are separated by __syncthreads (5 per plane); inside the Y phase warps are autonomous.
+//   * for one k1, x stage 2, the y work of 4 row pairs and the first x stage of the way back touch the same 4 pair
+//     storages and nothing else: a warp runs such a chain with __syncwarp only, so a plane needs 3 __syncthreads
+//     (after the first and before/after the last pruned radix-AX stage) and warps drift apart inside the chains,
+//     which lets the FP64 pipe of one overlap the shared-memory traffic of another.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -161,150 +164,160 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
         }
         __syncthreads();
 
-        // ------ X-inv stage 2: twiddle (warp-uniform) + radix-8, in place; lanes over 32 columns ------
-        for (int wi = warp; wi < (W2 / 32) * AX; wi += NW) {
-            const int grp = wi / AX, k1 = wi % AX;
-            const int cc = 32 * grp + lane0;
-            cplx* Zt = Z + k1 * PS;
-            cplx vv[8];
-#pragma unroll
-            for (int n2 = 0; n2 < 8; ++n2) vv[n2] = Zt[C::xrow(n2) + (cc ^ n2)];
-#pragma unroll
-            for (int n2 = 1; n2 < 8; ++n2) {
-                const cplx w = c_tw[OFFX + n2 * k1];
-                vv[n2] = cmul(vv[n2], w.x, w.y);
-            }
-            Dft<8, +1>::run(vv);
-            const double sgn = (32 * grp >= NKY0) ? -1.0 : 1.0;  // -ky columns hold the conjugate
-#pragma unroll
-            for (int k2 = 0; k2 < 8; ++k2) Zt[C::xrow(k2) + (cc ^ k2)] = cmake(vv[k2].x, sgn * vv[k2].y);
-        }
-        __syncthreads();
-        // now Z[m][cc] sits at pair storage (m % NPAIR), half (m / NPAIR), column cc ^ (m / AX)
-
-        // ------ Y: two row pairs (m, m + NX/2) per warp pass; Y3 on the pairs of two passes ------
+        // ------ chains: everything between the two pruned radix-AX stages touches, for one k1 (= n1), only the
+        // pair storages k1 + AX j (j < 4): x stage 2 (rows k1 + AX n2), the y transforms and the bracket of those
+        // 4 pairs, and the first x stage of the way back.  A warp runs whole chains; only __syncwarp inside ------
         {
             const int lane = opaque(lane0);
-            // Y2 item of this lane: pair pidx2 of the pass, k1 = k1y.  Lanes with (lane & 15) >= AY shadow item
-            // k1 = 0 (same addresses: broadcast) and only skip the final stores, so the phase has no divergent region
+            // Y2 item of this lane: pair pidx2 of the pass, k1 = k1y.  Lanes with (lane & 15) >= AY shadow an item
+            // of their own quarter-warp (same addresses: broadcast) and only skip the final stores, so the phase
+            // has no divergent region
             const int pidx2 = lane >> 4;
             const bool act2 = (lane & 15) < AY;
-            const int k1y = act2 ? (lane & 15) : 0;
+            const int k1y = act2 ? (lane & 15) : 8 + (lane & 3);
             cplx tq[8];  // W_NY^{k1y k2}: twiddles of this lane's Y2 items (inverse rows; conjugated on the way back)
 #pragma unroll
             for (int k2 = 1; k2 < 8; ++k2) tq[k2] = twy[k1y * 9 + k2];
-            int uprev = -1;
-            for (int u = warp; u < NPAIR / 2; u += NW) {
-                // chi values of this lane's Y2 item, requested now so that their latency hides behind Y1
-                const int pair2 = 2 * u + pidx2;
+
+            for (int c = warp; c < AX; c += NW) {
+                cplx* Zc = Z + c * PS;  // pair storage c; pair c + AX j is j*AX*PS further
+                // chi values of the first Y2 pass, requested now: their latency hides behind x stage 2 and Y1
                 cplx chv[2][8];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    const cplx* Rr = Rc + (size_t)(pair2 + h * NPAIR) * NY + k1y;
+                    const cplx* Rr = Rc + (size_t)(c + AX * pidx2 + h * NPAIR) * NY + k1y;
 #pragma unroll
                     for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc_early(Rr + AY * k2);
                 }
-                {  // Y1: pruned radix-AY, 4 rows x 8 lanes
-                    const int ridx = lane >> 3, n2 = lane & 7;
-                    const int pair1 = 2 * u + (ridx >> 1), h1 = ridx & 1;
-                    const int sw = (pair1 + h1 * NPAIR) / AX;  // column swizzle of this row
-                    const cplx* Zr = Z + pair1 * PS + h1 * W2 + (n2 ^ sw);
-                    cplx lo[AY1], hi[AY1];
+                // -- x stage 2: twiddle (warp-uniform) + radix-8, in place; lanes over 32 columns --
+                {
+                    cplx vv[W2 / 32][8];
 #pragma unroll
-                    for (int a = 0; a < AY1; ++a) {
-                        lo[a] = Zr[8 * a];
-                        hi[a] = Zr[8 * a + NKY0];
+                    for (int grp = 0; grp < W2 / 32; ++grp) {
+                        const int cc = 32 * grp + lane;
+#pragma unroll
+                        for (int n2 = 0; n2 < 8; ++n2) vv[grp][n2] = Zc[C::xrow(n2) + (cc ^ n2)];
                     }
-                    cplx out[AY];
-                    dft_pruned_in<AY, +1>(lo, hi, out);
-                    __syncwarp(FULL);  // every lane has read its row before the tiles overwrite the pair storage
-                    cplx* tile = (h1 ? ST + (warp * 2 + (ridx >> 1)) * FY : Z + pair1 * PS) + n2;
 #pragma unroll
-                    for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
-                }
-                __syncwarp(FULL);
-                {  // Y2: twiddle, to real space (both rows), bracket, back; result replaces tile 0 in place
-                    cplx* tile0 = Z + pair2 * PS + k1y * 9;
-                    const cplx* tile1 = ST + (warp * 2 + pidx2) * FY + k1y * 9;
-                    cplx v0[8], v1[8];
+                    for (int grp = 0; grp < W2 / 32; ++grp) {
+                        const int cc = 32 * grp + lane;
 #pragma unroll
-                    for (int n2 = 0; n2 < 8; ++n2) v0[n2] = tile0[n2];
+                        for (int n2 = 1; n2 < 8; ++n2) {
+                            const cplx w = c_tw[OFFX + n2 * c];
+                            vv[grp][n2] = cmul(vv[grp][n2], w.x, w.y);
+                        }
+                        Dft<8, +1>::run(vv[grp]);
+                        const double sgn = (32 * grp >= NKY0) ? -1.0 : 1.0;  // -ky columns hold the conjugate
 #pragma unroll
-                    for (int n2 = 0; n2 < 8; ++n2) v1[n2] = tile1[n2];
-#pragma unroll
-                    for (int n2 = 1; n2 < 8; ++n2) {
-                        v0[n2] = cmul(v0[n2], tq[n2].x, tq[n2].y);
-                        v1[n2] = cmul(v1[n2], tq[n2].x, tq[n2].y);
-                    }
-                    Dft<8, +1>::run(v0);
-                    Dft<8, +1>::run(v1);
-                    cplx w[8];
-#pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) {  // dx chi * dy g - dy chi * dx g for rows m and m + NX/2
-                        w[k2].x = fma(chv[0][k2].x, v0[k2].y, -chv[0][k2].y * v0[k2].x);
-                        w[k2].y = fma(chv[1][k2].x, v1[k2].y, -chv[1][k2].y * v1[k2].x);
-                    }
-                    Dft<8, -1>::run(w);
-#pragma unroll
-                    for (int k2 = 1; k2 < 8; ++k2) w[k2] = cmul(w[k2], tq[k2].x, -tq[k2].y);
-                    __syncwarp(FULL);  // shadow lanes have read tile 0 of k1 = 0 before lane 0 overwrites it
-                    if (act2) {
-#pragma unroll
-                        for (int k2 = 0; k2 < 8; ++k2) tile0[k2] = w[k2];
+                        for (int k2 = 0; k2 < 8; ++k2)
+                            Zc[C::xrow(k2) + (cc ^ k2)] = cmake(vv[grp][k2].x, sgn * vv[grp][k2].y);
                     }
                 }
                 __syncwarp(FULL);
-                const bool both = uprev >= 0;
-                if (both || u + NW >= NPAIR / 2) {
-                    // Y3: pruned-output radix-AY on the pairs of this pass (lanes 16-31) and of the previous one
-                    // (lanes 0-15); P[pair][cc] overwrites tile 0 after everyone has read it
-                    const bool act3 = both || lane >= 16;
-                    const int pair3 = 2 * ((lane >> 4) ? u : uprev) + ((lane >> 3) & 1), k2 = lane & 7;
-                    cplx in[AY];
-                    if (act3) {
+                // now Z[m][cc], m = c + AX k2, sits in pair storage c + AX (k2 & 3), half k2 >> 2, column cc ^ k2
+
+                // -- y: pass 0 on pairs c, c + AX; pass 1 on pairs c + 2 AX, c + 3 AX --
+#pragma unroll 1
+                for (int pass = 0; pass < 2; ++pass) {
+                    if (pass) {
 #pragma unroll
-                        for (int n1 = 0; n1 < AY; ++n1) in[n1] = Z[pair3 * PS + n1 * 9 + k2];
-                    }
-                    __syncwarp(FULL);
-                    if (act3) {
-                        cplx lo[AY1], hi[AY1];
-                        dft_pruned_out<AY, -1>(in, lo, hi);
-                        cplx* Pp = Z + pair3 * PS + k2;
+                        for (int h = 0; h < 2; ++h) {
+                            const cplx* Rr = Rc + (size_t)(c + AX * (2 + pidx2) + h * NPAIR) * NY + k1y;
 #pragma unroll
-                        for (int c = 0; c < AY1; ++c) {
-                            Pp[8 * c] = lo[c];
-                            Pp[8 * c + NKY0] = hi[c];
+                            for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc_early(Rr + AY * k2);
                         }
                     }
-                    uprev = -1;
-                } else {
-                    uprev = u;
+                    {  // Y1: pruned radix-AY, 4 rows x 8 lanes
+                        const int ridx = lane >> 3, n2 = lane & 7;
+                        const int j1 = 2 * pass + (ridx >> 1), h1 = ridx & 1;
+                        const int sw = j1 + 4 * h1;  // column swizzle of row c + AX (j1 + 4 h1)
+                        const cplx* Zr = Zc + j1 * (AX * PS) + h1 * W2 + (n2 ^ sw);
+                        cplx lo[AY1], hi[AY1];
+#pragma unroll
+                        for (int a = 0; a < AY1; ++a) {
+                            lo[a] = Zr[8 * a];
+                            hi[a] = Zr[8 * a + NKY0];
+                        }
+                        cplx out[AY];
+                        dft_pruned_in<AY, +1>(lo, hi, out);
+                        __syncwarp(FULL);  // every lane has read its row before the tiles overwrite the pair storage
+                        cplx* tile = (h1 ? ST + (warp * 2 + (ridx >> 1)) * FY : Zc + j1 * (AX * PS)) + n2;
+#pragma unroll
+                        for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
+                    }
+                    __syncwarp(FULL);
+                    {  // Y2: twiddle, to real space (both rows), bracket, back; result replaces tile 0 in place
+                        cplx* tile0 = Zc + (2 * pass + pidx2) * (AX * PS) + k1y * 9;
+                        const cplx* tile1 = ST + (warp * 2 + pidx2) * FY + k1y * 9;
+                        cplx v0[8], v1[8];
+#pragma unroll
+                        for (int n2 = 0; n2 < 8; ++n2) v0[n2] = tile0[n2];
+#pragma unroll
+                        for (int n2 = 0; n2 < 8; ++n2) v1[n2] = tile1[n2];
+#pragma unroll
+                        for (int n2 = 1; n2 < 8; ++n2) {
+                            v0[n2] = cmul(v0[n2], tq[n2].x, tq[n2].y);
+                            v1[n2] = cmul(v1[n2], tq[n2].x, tq[n2].y);
+                        }
+                        Dft<8, +1>::run(v0);
+                        Dft<8, +1>::run(v1);
+                        cplx w[8];
+#pragma unroll
+                        for (int k2 = 0; k2 < 8; ++k2) {  // dx chi * dy g - dy chi * dx g for rows m and m + NX/2
+                            w[k2].x = fma(chv[0][k2].x, v0[k2].y, -chv[0][k2].y * v0[k2].x);
+                            w[k2].y = fma(chv[1][k2].x, v1[k2].y, -chv[1][k2].y * v1[k2].x);
+                        }
+                        Dft<8, -1>::run(w);
+#pragma unroll
+                        for (int k2 = 1; k2 < 8; ++k2) w[k2] = cmul(w[k2], tq[k2].x, -tq[k2].y);
+                        __syncwarp(FULL);  // shadow lanes have read their tiles before the owners overwrite them
+                        if (act2) {
+#pragma unroll
+                            for (int k2 = 0; k2 < 8; ++k2) tile0[k2] = w[k2];
+                        }
+                    }
+                    __syncwarp(FULL);
                 }
-            }
-        }
-        __syncthreads();
+                {  // Y3: pruned-output radix-AY on the 4 pairs; P[pair][cc] overwrites tile 0 after everyone has read it
+                    const int k2 = lane & 7;
+                    cplx* Pp = Zc + (lane >> 3) * (AX * PS) + k2;
+                    cplx in[AY];
+#pragma unroll
+                    for (int n1 = 0; n1 < AY; ++n1) in[n1] = Pp[n1 * 9];
+                    __syncwarp(FULL);
+                    cplx lo[AY1], hi[AY1];
+                    dft_pruned_out<AY, -1>(in, lo, hi);
+#pragma unroll
+                    for (int cq = 0; cq < AY1; ++cq) {
+                        Pp[8 * cq] = lo[cq];
+                        Pp[8 * cq + NKY0] = hi[cq];
+                    }
+                }
+                __syncwarp(FULL);
 
-        // ------ X-fwd stage 1: unpack the row pair, radix-8, twiddle (warp-uniform); lanes over 32 columns ------
-        // tile slot (kyi, n1, k2) goes to the free second half of pair storage n1 + AX (k2 & 3)
-        for (int wi = warp; wi < (NKY0 / 32) * AX; wi += NW) {
-            const int kg = wi / AX, n1 = wi % AX;
-            const int kyi = 32 * kg + lane0;
-            const cplx* Pp = Z + n1 * PS + kyi;
-            const cplx* Pm = Z + n1 * PS + (kyi ? W2 - kyi : 0);
-            cplx xx[8];
+                // -- x stage 1 of the way back: unpack the row pair, radix-8, twiddle (warp-uniform); lanes over 32
+                // columns.  Tile slot (kyi, n1 = c, k2) goes to the free second half of pair storage c + AX (k2 & 3) --
 #pragma unroll
-            for (int n2 = 0; n2 < 4; ++n2) {  // rows m = n1 + AX n2 and m + NX/2 of pair n1 + AX n2
-                const cplx pp = Pp[AX * n2 * PS], pm = Pm[AX * n2 * PS];
-                xx[n2] = cmake(pp.x + pm.x, pp.y - pm.y);      // 2 N^_m  = P+ + conj P-
-                xx[n2 + 4] = cmake(pp.y + pm.y, pm.x - pp.x);  // 2 N^_m' = -i (P+ - conj P-)
-            }
-            Dft<8, -1>::run(xx);
-            cplx* Zt = Z + n1 * PS + W2;
-            Zt[kyi] = xx[0];
+                for (int kg = 0; kg < NKY0 / 32; ++kg) {
+                    const int kyi = 32 * kg + lane;
+                    const cplx* Pq = Zc + kyi;
+                    const cplx* Pm = Zc + (kyi ? W2 - kyi : 0);
+                    cplx xx[8];
 #pragma unroll
-            for (int k2 = 1; k2 < 8; ++k2) {
-                const cplx w = c_tw[OFFX + n1 * k2];
-                Zt[(AX * (k2 & 3)) * PS + NKY0 * (k2 >> 2) + (kyi ^ k2)] = cmul(xx[k2], w.x, -w.y);
+                    for (int n2 = 0; n2 < 4; ++n2) {  // rows m = c + AX n2 and m + NX/2 of pair c + AX n2
+                        const cplx pp = Pq[AX * n2 * PS], pm = Pm[AX * n2 * PS];
+                        xx[n2] = cmake(pp.x + pm.x, pp.y - pm.y);      // 2 N^_m  = P+ + conj P-
+                        xx[n2 + 4] = cmake(pp.y + pm.y, pm.x - pp.x);  // 2 N^_m' = -i (P+ - conj P-)
+                    }
+                    Dft<8, -1>::run(xx);
+                    cplx* Zt = Zc + W2;
+                    Zt[kyi] = xx[0];
+#pragma unroll
+                    for (int k2 = 1; k2 < 8; ++k2) {
+                        const cplx w = c_tw[OFFX + c * k2];
+                        Zt[(AX * (k2 & 3)) * PS + NKY0 * (k2 >> 2) + (kyi ^ k2)] = cmul(xx[k2], w.x, -w.y);
+                    }
+                }
             }
         }
         __syncthreads();
