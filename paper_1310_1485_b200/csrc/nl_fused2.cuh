@@ -89,24 +89,55 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
     load_twiddles_ab<AY, 8>(twy, twy_g);
     __syncthreads();
 
+    static_assert(NKY0 / 4 == NW, "one pruned radix-AX pass (4 stored columns) per warp");
     const long long T = (long long)nslab * nz * nv;
     const size_t plane_elems = (size_t)NX0 * NKY0;
+    // planes are walked v-fastest so that neighbouring CTAs share a chi plane in L2
+    auto plane_of = [&](long long tt) {
+        const int v = (int)(tt % nv);
+        const int z = (int)((tt / nv) % nz);
+        const long long sl = tt / ((long long)nv * nz);
+        return (size_t)z + (size_t)nz * ((size_t)v + (size_t)nv * sl);
+    };
+    // This warp's share of a spectral plane for the first x stage (column kyi = 4 warp + lane/8, rows n2 + 8a and
+    // n2 + 8a + M).  Requested one barrier ahead of its use: for the first plane here, for later planes at the end of
+    // the previous one, so that the L2 latency hides behind the warps that are still working.
+    cplx f0[AX1], f1[AX1];
+    auto request_g = [&](long long tt) {
+        const int lane = opaque(lane0);
+        const int n2 = lane & 7, kyi = 4 * warp + (lane >> 3);
+        const cplx* F = g + plane_of(tt) * plane_elems;
+        const cplx* Fc = F + (size_t)kyi * NX0 + n2;
+#pragma unroll
+        for (int a = 0; a < AX1; ++a) {
+#ifdef GNL_EXP_NOG
+            f0[a] = cmake(n2 + a, kyi); f1[a] = cmake(kyi, a);
+#else
+            f0[a] = ldg_nc_early(Fc + 8 * a);
+            f1[a] = ldg_nc_early(Fc + 8 * a + M);
+#endif
+        }
+        if (kyi == 0) {  // Hermitian part of the ky = 0 column (reading R7)
+#pragma unroll
+            for (int a = 0; a < AX1; ++a) {
+                const int i0 = n2 + 8 * a, i1 = i0 + M;
+                const cplx m0 = F[(NX0 - i0) % NX0], m1 = F[NX0 - i1];
+                f0[a] = cmake(0.5 * (f0[a].x + m0.x), 0.5 * (f0[a].y - m0.y));
+                f1[a] = cmake(0.5 * (f1[a].x + m1.x), 0.5 * (f1[a].y - m1.y));
+            }
+        }
+        if (n2 == 0) f1[0] = cmake(0.0, 0.0);  // i = M: the Nyquist row is ignored (R6)
+    };
+    if ((long long)blockIdx.x < T) request_g(blockIdx.x);
     for (long long t = blockIdx.x; t < T; t += gridDim.x) {
-        // planes are walked v-fastest so that neighbouring CTAs share a chi plane in L2
-        const int v = (int)(t % nv);
-        const int z = (int)((t / nv) % nz);
-        const long long sl = t / ((long long)nv * nz);
-        const size_t p = (size_t)z + (size_t)nz * ((size_t)v + (size_t)nv * sl);
-        const size_t q = chi_has_v ? p : (size_t)z + (size_t)nz * sl;
-        const cplx* F = g + p * plane_elems;
+        const size_t p = plane_of(t);
+        const size_t q = chi_has_v ? p : (size_t)((t / nv) % nz) + (size_t)nz * (size_t)(t / ((long long)nv * nz));
         cplx* Rb = rhs + p * plane_elems;
         const cplx* Rc = R + q * ((size_t)NX * NY);
         {  // pull the next plane's g and rhs towards L2 while this one is being worked on
             const long long tn = t + gridDim.x;
             if (tn < T) {
-                const int vn = (int)(tn % nv), zn = (int)((tn / nv) % nz);
-                const long long sn = tn / ((long long)nv * nz);
-                const size_t pn = (size_t)zn + (size_t)nz * ((size_t)vn + (size_t)nv * sn);
+                const size_t pn = plane_of(tn);
                 const char* a = (const char*)(g + pn * plane_elems);
                 const char* b = (const char*)(rhs + pn * plane_elems);
                 for (size_t off = (size_t)threadIdx.x * 128; off < plane_elems * sizeof(cplx); off += (size_t)NW * 32 * 128) {
@@ -116,27 +147,10 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
             }
         }
 
-        // ------ X-inv stage 1: derivative, pad, pruned radix-AX; 4 stored columns x 8 n2 per warp pass ------
-        for (int u = warp; u < NKY0 / 4; u += NW) {
+        // ------ X-inv stage 1: derivative, pad, pruned radix-AX; 4 stored columns x 8 n2 per warp ------
+        {
             const int lane = opaque(lane0);
-            const int n2 = lane & 7, kyi = 4 * u + (lane >> 3);
-            const cplx* Fc = F + (size_t)kyi * NX0 + n2;
-            cplx f0[AX1], f1[AX1];
-#pragma unroll
-            for (int a = 0; a < AX1; ++a) {
-                f0[a] = Fc[8 * a];
-                f1[a] = Fc[8 * a + M];
-            }
-            if (kyi == 0) {  // Hermitian part of the ky = 0 column (reading R7)
-#pragma unroll
-                for (int a = 0; a < AX1; ++a) {
-                    const int i0 = n2 + 8 * a, i1 = i0 + M;
-                    const cplx m0 = F[(NX0 - i0) % NX0], m1 = F[NX0 - i1];
-                    f0[a] = cmake(0.5 * (f0[a].x + m0.x), 0.5 * (f0[a].y - m0.y));
-                    f1[a] = cmake(0.5 * (f1[a].x + m1.x), 0.5 * (f1[a].y - m1.y));
-                }
-            }
-            if (n2 == 0) f1[0] = cmake(0.0, 0.0);  // i = M: the Nyquist row is ignored (R6)
+            const int n2 = lane & 7, kyi = 4 * warp + (lane >> 3);
             const double ky = kymin * (double)kyi, dn2 = (double)n2;
             cplx* Zl = Z + C::xrow(n2);
 #pragma unroll 1
@@ -187,7 +201,11 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                 for (int h = 0; h < 2; ++h) {
                     const cplx* Rr = Rc + (size_t)(c + AX * pidx2 + h * NPAIR) * NY + k1y;
 #pragma unroll
+#ifdef GNL_EXP_NOCHI
+                    for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = cmake(k2 + h, lane);
+#else
                     for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc_early(Rr + AY * k2);
+#endif
                 }
                 // -- x stage 2: twiddle (warp-uniform) + radix-8, in place; lanes over 32 columns --
                 {
@@ -224,7 +242,11 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                         for (int h = 0; h < 2; ++h) {
                             const cplx* Rr = Rc + (size_t)(c + AX * (2 + pidx2) + h * NPAIR) * NY + k1y;
 #pragma unroll
+#ifdef GNL_EXP_NOCHI
+                            for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = cmake(k2 + h, lane + (size_t)Rr % 3);
+#else
                             for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc_early(Rr + AY * k2);
+#endif
                         }
                     }
                     {  // Y1: pruned radix-AY, 4 rows x 8 lanes
@@ -320,19 +342,29 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                 }
             }
         }
-        __syncthreads();
-
-        // ------ X-fwd stage 2: pruned-output radix-AX, delete modes, prefactor, add; 4 columns x 8 k2 per pass ------
-        for (int u = warp; u < NKY0 / 4; u += NW) {
+        // rhs values of this warp's share of the last stage, requested ahead of the barrier: the warps that finish
+        // their chains first hide the latency behind the others
+        cplx r0[AX1], r1[AX1];
+        {
             const int lane = opaque(lane0);
-            const int k2 = lane & 7, kyi = 4 * u + (lane >> 3);
-            cplx* Rcol = Rb + (size_t)kyi * NX0 + k2;
-            cplx r0[AX1], r1[AX1];
+            const cplx* Rcol = Rb + (size_t)(4 * warp + (lane >> 3)) * NX0 + (lane & 7);
 #pragma unroll
-            for (int c = 0; c < AX1; ++c) {  // requested early: the latency hides behind the butterfly
+            for (int c = 0; c < AX1; ++c) {
+#ifdef GNL_EXP_NORHS
+                r0[c] = cmake(1, 2); r1[c] = cmake(3, 4);
+#else
                 r0[c] = ldg_early(Rcol + 8 * c);
                 r1[c] = ldg_early(Rcol + 8 * c + M);
+#endif
             }
+        }
+        __syncthreads();
+
+        // ------ X-fwd stage 2: pruned-output radix-AX, delete modes, prefactor, add; 4 columns x 8 k2 per warp ------
+        {
+            const int lane = opaque(lane0);
+            const int k2 = lane & 7, kyi = 4 * warp + (lane >> 3);
+            cplx* Rcol = Rb + (size_t)kyi * NX0 + k2;
             const cplx* Zt = Z + W2 + (AX * (k2 & 3)) * PS + NKY0 * (k2 >> 2) + (kyi ^ k2);
             cplx in[AX];
 #pragma unroll
@@ -346,6 +378,7 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                     Rcol[8 * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
             }
         }
+        if (t + gridDim.x < T) request_g(t + gridDim.x);
         __syncthreads();
     }
 }
