@@ -359,6 +359,8 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
             }
         }
         __syncthreads();
+        // next plane's share of g, requested here: the last x stage and the rhs update hide its latency
+        if (t + gridDim.x < T) request_g(t + gridDim.x);
 
         // ------ X-fwd stage 2: pruned-output radix-AX, delete modes, prefactor, add; 4 columns x 8 k2 per warp ------
         {
@@ -378,7 +380,6 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                     Rcol[8 * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
             }
         }
-        if (t + gridDim.x < T) request_g(t + gridDim.x);
         __syncthreads();
     }
 }

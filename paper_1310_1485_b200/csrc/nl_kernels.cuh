@@ -201,7 +201,7 @@ k_yreal(const cplx* __restrict__ Z, cplx* __restrict__ R, const cplx* __restrict
 template <int NY, int A, int B, int RP, int NT>
 __global__ void __launch_bounds__(NT)
 k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restrict__ P,
-           const cplx* __restrict__ tw_g, int Nx, int nzb, int chi_per_plane)
+           const cplx* __restrict__ tw_g, int Nx, int nzb, int chi_per_plane, int vfast)
 {
     constexpr int A1 = A / 3, NKY0 = NY / 3, W2 = 2 * NKY0;
     constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
@@ -210,8 +210,17 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
     cplx* E = smem + RS;
     const int half = Nx / 2;
     const int ntile = half / RP;
-    const int bl = blockIdx.x / ntile;
-    const int m0 = (blockIdx.x % ntile) * RP;
+    int bl, m0;
+    if (vfast) {
+        // CTAs numbered v-fastest: neighbours in launch order work on the same rows of the same chi plane (one z,
+        // all v of the batch), so chi rows too large to stay in L2 are fetched from HBM once per batch
+        const int nvc = gridDim.x / (ntile * nzb);
+        m0 = ((blockIdx.x / nvc) % ntile) * RP;
+        bl = blockIdx.x / (nvc * ntile) + nzb * (blockIdx.x % nvc);
+    } else {
+        bl = blockIdx.x / ntile;
+        m0 = (blockIdx.x % ntile) * RP;
+    }
     const int ql = chi_per_plane ? bl : bl % nzb;
     load_twiddles_ab<A, B>(tw, tw_g);
     __syncthreads();
