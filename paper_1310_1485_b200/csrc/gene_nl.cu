@@ -132,7 +132,7 @@ YKernels make_y()
 {
     YKernels k;
     k.ny = NY; k.rp = RP; k.rt = 2 * RP; k.nt = NT;
-    k.smem_br = sizeof(cplx) * (size_t)((1 + 2 * RP) * gnl::Tile<A, B>::FLAT);
+    k.smem_br = sizeof(cplx) * (size_t)(2 * RP * gnl::Tile<A, B>::FLAT);  // exchange tiles only (twiddles come through L1)
     k.smem_real = k.smem_br;
     k.br = gnl::k_ybracket<NY, A, B, RP, NT>;
     k.real = gnl::k_yreal<NY, A, B, 2 * RP, NT>;

@@ -21,6 +21,12 @@
 
 #include "dft_regs.cuh"
 
+// Twiddle W_N^{i j} of a two-stage transform.  The x kernels read it from a padded shared-memory table filled in the
+// CTA prologue; the y kernels read the global table through L1 (no prologue, no barrier before the first row load):
+// measured on B200, that is faster for k_yreal / k_ybracket (-16 % at 144x144) and slower for k_xinv / k_xfwd.
+#define TWD(i, j) tw[(i) * BP + (j)]
+#define TWD_G(i, j) __ldg(reinterpret_cast<const double2*>(tw_g) + (i) * (j))
+
 namespace gnl {
 
 __host__ __device__ constexpr int odd_up(int v) { return v | 1; }
@@ -110,7 +116,7 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
         cplx* Ec = E + c2 * CS + n2;
 #pragma unroll
         for (int k1 = 0; k1 < A; ++k1) {
-            cplx w = tw[k1 * BP + n2];
+            cplx w = TWD(k1, n2);
             Ec[k1 * BP] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
         }
     }
@@ -141,7 +147,7 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
 // stage 1 of the y-synthesis, shared by k_yreal and k_ybracket: rows of Z -> exchange tile
 // ------------------------------------------------------------------------------------------------
 template <int NY, int A, int B>
-__device__ __forceinline__ void y_stage1(const cplx* __restrict__ Zr, const cplx* tw, cplx* Er, int n2)
+__device__ __forceinline__ void y_stage1(const cplx* __restrict__ Zr, const cplx* __restrict__ tw_g, cplx* Er, int n2)
 {
     constexpr int A1 = A / 3, NKY0 = NY / 3, BP = Tile<A, B>::BP;
     cplx lo[A1], hi[A1];
@@ -154,7 +160,7 @@ __device__ __forceinline__ void y_stage1(const cplx* __restrict__ Zr, const cplx
     dft_pruned_in<A, +1>(lo, hi, out);
 #pragma unroll
     for (int k1 = 0; k1 < A; ++k1) {
-        cplx w = tw[k1 * BP + n2];
+        cplx w = TWD_G(k1, n2);
         Er[k1 * BP + n2] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
     }
 }
@@ -169,16 +175,13 @@ k_yreal(const cplx* __restrict__ Z, cplx* __restrict__ R, const cplx* __restrict
     constexpr int W2 = 2 * (NY / 3);
     constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
     extern __shared__ cplx smem[];
-    cplx* tw = smem;
-    cplx* E = smem + RS;
+    cplx* E = smem;
     const int ntile = Nx / RT;
     const int ql = blockIdx.x / ntile;
     const int m0 = (blockIdx.x % ntile) * RT;
-    load_twiddles_ab<A, B>(tw, tw_g);
-    __syncthreads();
     for (int item = threadIdx.x; item < RT * B; item += NT) {
         const int n2 = item % B, r = item / B;
-        y_stage1<NY, A, B>(Z + ((size_t)ql * Nx + m0 + r) * W2, tw, E + r * RS, n2);
+        y_stage1<NY, A, B>(Z + ((size_t)ql * Nx + m0 + r) * W2, tw_g, E + r * RS, n2);
     }
     __syncthreads();
     for (int item = threadIdx.x; item < RT * A; item += NT) {
@@ -206,8 +209,7 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
     constexpr int A1 = A / 3, NKY0 = NY / 3, W2 = 2 * NKY0;
     constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
     extern __shared__ cplx smem[];
-    cplx* tw = smem;
-    cplx* E = smem + RS;
+    cplx* E = smem;
     const int half = Nx / 2;
     const int ntile = half / RP;
     int bl, m0;
@@ -222,14 +224,12 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
         m0 = (blockIdx.x % ntile) * RP;
     }
     const int ql = chi_per_plane ? bl : bl % nzb;
-    load_twiddles_ab<A, B>(tw, tw_g);
-    __syncthreads();
 
     // Y1: pruned radix-A + twiddle for the 2*RP rows of the tile
     for (int item = threadIdx.x; item < 2 * RP * B; item += NT) {
         const int n2 = item % B, r = item / B;
         const int m = m0 + (r % RP) + (r / RP) * half;
-        y_stage1<NY, A, B>(Z + ((size_t)bl * Nx + m) * W2, tw, E + r * RS, n2);
+        y_stage1<NY, A, B>(Z + ((size_t)bl * Nx + m) * W2, tw_g, E + r * RS, n2);
     }
     __syncthreads();
 
@@ -258,7 +258,7 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
         cplx* Er = E + r * RS + k1 * BP;
 #pragma unroll
         for (int k2 = 0; k2 < B; ++k2) {
-            cplx t = tw[k1 * BP + k2];
+            cplx t = TWD_G(k1, k2);
             Er[k2] = (k2 == 0) ? w[0] : cmul(w[k2], t.x, -t.y);
         }
     }
@@ -322,7 +322,7 @@ k_xfwd(const cplx* __restrict__ P, cplx* __restrict__ rhs, const cplx* __restric
         cplx* Ec = E + col * CS + n1 * BP;
 #pragma unroll
         for (int k2 = 0; k2 < B; ++k2) {
-            cplx t = tw[n1 * BP + k2];
+            cplx t = TWD(n1, k2);
             Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], t.x, -t.y);
         }
     }
