@@ -12,5 +12,7 @@ from .gene_nl_oracle import (  # noqa: F401
     nl_convolution_modes,
     nl_convolution_plane,
     nl_pseudospectral,
+    nlx_convolution_plane,
+    nlx_pseudospectral,
     num_threads,
 )

@@ -262,3 +262,99 @@ void oracle_nl_convolution_modes(int nx0, int nky0, double kxmin, double kymin,
         out[t] = convolution_mode(nx0, nky0, kxmin, kymin, (const cplx *)chi_ri, (const cplx *)g_ri, a, j);
     }
 }
+
+/* =====================================================================================================
+ * x-GLOBAL VARIANT -- the operator the paper itself ran and timed.
+ *
+ * PAPER.md:39 (sect. 2): GENE's x-global version is spectral in y only; "the fields are
+ * preprocessed (transposition, extension in y direction for dealiasing according to the 3/2-rule) in a
+ * first step, and a fast Fourier transform to real space is applied.  After multiplication the result is
+ * transformed back to the spectral representation, the additional modes are deleted, the array is
+ * transposed and multiplied with a prefactor, and is finally added to the right-hand side vector."
+ * "The nonlinear term needs as input four arrays, the x and y component of the ExB-velocity
+ * and the derivatives of the distribution function with respect to x and y.  Additionally it needs the
+ * already computed right-hand side" (5 planes in, 1 out: intensity 1/6).
+ *
+ * A plane is nx*nky0 complex128, x fastest: F[x + nx*j], x a REAL-SPACE point, j the ky index
+ * (ky >= 0; ky < 0 implied by reality of the field; Im F[x,0] is ignored, as in reading R7).
+ * Per plane and per x:   N(x,y) = vex(x,y)*dxg(x,y) + vey(x,y)*dyg(x,y)   (v_E . grad g) on the padded
+ * real grid Ny = 3*nky0, and   rhs[x,j] += scale * pref[x] * N^(x,j),  j < nky0,  N^ = (1/Ny) sum_y N e^{-i..}.
+ * Readings (the paper gives no formulas): the sign and any metric factor live in pref/scale; pref is a
+ * real array over x ("prefactor", x-dependent in an x-global code); Ny = 3*nky0 as in R8.
+ * Two routes, as above: the definition (truncated convolution over ky) and the algorithm step by step.
+ * ===================================================================================================== */
+
+/* Hermitian extension in ky of the stored half-spectrum at one x: b in (-nky0, nky0) */
+static cplx extx_mode(const cplx *F, int nx, int x, int b)
+{
+    if (b == 0) return creal(F[x]);
+    if (b > 0) return F[x + (long)nx * b];
+    return conj(F[x + (long)nx * (-b)]);
+}
+
+/* (1) THE DEFINITION: N^(x,k) = sum_{k'+k''=k, |k'|,|k''| < nky0} [vex(k') dxg(k'') + vey(k') dyg(k'')] */
+void oracle_nlx_convolution_plane(int nx, int nky0, const double *vex_ri, const double *vey_ri,
+                                  const double *dxg_ri, const double *dyg_ri, double *out_ri)
+{
+    const cplx *vex = (const cplx *)vex_ri, *vey = (const cplx *)vey_ri;
+    const cplx *dxg = (const cplx *)dxg_ri, *dyg = (const cplx *)dyg_ri;
+    cplx *out = (cplx *)out_ri;
+    for (int x = 0; x < nx; ++x)
+        for (int k = 0; k < nky0; ++k) {
+            cplx acc = 0.0;
+            for (int k1 = -(nky0 - 1); k1 <= nky0 - 1; ++k1) {
+                int k2 = k - k1;
+                if (k2 <= -nky0 || k2 >= nky0) continue;
+                acc += extx_mode(vex, nx, x, k1) * extx_mode(dxg, nx, x, k2) +
+                       extx_mode(vey, nx, x, k1) * extx_mode(dyg, nx, x, k2);
+            }
+            out[x + (long)nx * k] = acc;
+        }
+}
+
+/* to real space at one x: extension to Ny = 3 nky0 (zero modes added), synthesis e^{+i ky y}, real part */
+static void nlx_to_real(int backend, int nx, int nky0, int Ny, const cplx *wp, const cplx *F, int x,
+                        cplx *S, cplx *T, double *f)
+{
+    for (int j = 0; j < Ny; ++j) S[j] = 0.0;
+    for (int j = 0; j < nky0; ++j) {
+        S[j] = F[x + (long)nx * j];
+        if (j >= 1) S[Ny - j] = conj(F[x + (long)nx * j]);
+    }
+    dft1d(backend, Ny, wp, S, 1, T);
+    for (int n = 0; n < Ny; ++n) f[n] = creal(T[n]);
+}
+
+/* (2) THE ALGORITHM of PAPER.md:61, plane by plane (OpenMP over planes) */
+void oracle_nlx_pseudospectral(int backend, int nx, int nky0, long planes, const double *vex_ri,
+                               const double *vey_ri, const double *dxg_ri, const double *dyg_ri,
+                               const double *pref, double *rhs_ri, double scale)
+{
+    const int Ny = 3 * nky0;
+    const long M = (long)nx * nky0;
+    cplx *wp = root_table(Ny, +1), *wm = root_table(Ny, -1);
+#pragma omp parallel
+    {
+        cplx *S = (cplx *)malloc(sizeof(cplx) * (size_t)Ny), *T = (cplx *)malloc(sizeof(cplx) * (size_t)Ny);
+        double *a = (double *)malloc(sizeof(double) * (size_t)Ny * 4);
+#pragma omp for schedule(static)
+        for (long p = 0; p < planes; ++p) {
+            const cplx *vex = (const cplx *)vex_ri + p * M, *vey = (const cplx *)vey_ri + p * M;
+            const cplx *dxg = (const cplx *)dxg_ri + p * M, *dyg = (const cplx *)dyg_ri + p * M;
+            cplx *rhs = (cplx *)rhs_ri + p * M;
+            for (int x = 0; x < nx; ++x) {
+                nlx_to_real(backend, nx, nky0, Ny, wp, vex, x, S, T, a);
+                nlx_to_real(backend, nx, nky0, Ny, wp, vey, x, S, T, a + Ny);
+                nlx_to_real(backend, nx, nky0, Ny, wp, dxg, x, S, T, a + 2 * Ny);
+                nlx_to_real(backend, nx, nky0, Ny, wp, dyg, x, S, T, a + 3 * Ny);
+                for (int n = 0; n < Ny; ++n) /* multiplication in real space */
+                    S[n] = a[n] * a[2 * Ny + n] + a[Ny + n] * a[3 * Ny + n];
+                dft1d(backend, Ny, wm, S, 1, T);                /* back to the spectral representation */
+                for (int j = 0; j < nky0; ++j)                  /* additional modes deleted, prefactor, add */
+                    rhs[x + (long)nx * j] += scale * pref[x] * (T[j] / (double)Ny);
+            }
+        }
+        free(S); free(T); free(a);
+    }
+    free(wp); free(wm);
+}

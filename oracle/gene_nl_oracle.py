@@ -53,6 +53,11 @@ def _load():
                 ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, dp, dp,
                 ctypes.c_int, ip, ip, dp]
             lib.oracle_nl_convolution_modes.restype = None
+            lib.oracle_nlx_convolution_plane.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp, dp, dp, dp]
+            lib.oracle_nlx_convolution_plane.restype = None
+            lib.oracle_nlx_pseudospectral.argtypes = [
+                ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_long, dp, dp, dp, dp, dp, dp, ctypes.c_double]
+            lib.oracle_nlx_pseudospectral.restype = None
             _lib = lib
     return _lib
 
@@ -136,3 +141,29 @@ def nl_convolution_modes(chi, g, kxmin: float, kymin: float, i_idx, j_idx) -> np
                                         int(ii.size), ii.ctypes.data_as(ip), jj.ctypes.data_as(ip),
                                         _dptr(out))
     return out
+
+
+# ---- x-global variant: planes of shape (nky0, nx), x fastest ----
+def nlx_convolution_plane(vex, vey, dxg, dyg) -> np.ndarray:
+    """N^(x, ky) = sum over ky' of [vex dxg + vey dyg] for ONE plane, by the definition (truncated convolution)."""
+    vex, vey, dxg, dyg = (_c128(a) for a in (vex, vey, dxg, dyg))
+    nky0, nx = vex.shape
+    out = np.zeros_like(vex)
+    _load().oracle_nlx_convolution_plane(nx, nky0, _dptr(vex), _dptr(vey), _dptr(dxg), _dptr(dyg), _dptr(out))
+    return out
+
+
+def nlx_pseudospectral(vex, vey, dxg, dyg, pref, rhs, scale: float, backend: int = DFT_RECURSIVE) -> np.ndarray:
+    """rhs + scale*pref[x]*N^ for a stack of planes (P, nky0, nx), by the algorithm of PAPER.md:61."""
+    vex, vey, dxg, dyg = (_c128(a) for a in (vex, vey, dxg, dyg))
+    out = _c128(rhs).copy()
+    single = vex.ndim == 2
+    if single:
+        vex, vey, dxg, dyg, out = vex[None], vey[None], dxg[None], dyg[None], out[None]
+    P, nky0, nx = vex.shape
+    assert all(a.shape == vex.shape for a in (vey, dxg, dyg, out))
+    pref = np.ascontiguousarray(pref, dtype=np.float64)
+    assert pref.shape == (nx,)
+    _load().oracle_nlx_pseudospectral(int(backend), nx, nky0, P, _dptr(vex), _dptr(vey), _dptr(dxg), _dptr(dyg),
+                                      _dptr(pref), _dptr(out), float(scale))
+    return out[0] if single else out
