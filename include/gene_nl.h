@@ -128,6 +128,40 @@ double gene_nl_query(const gene_nl_plan* h, int what);
  */
 int gene_nl_probe_peaks(double* out3);
 
+/* =====================================================================================================
+ * x-GLOBAL VARIANT -- the operator the paper itself ran and timed (PAPER.md:39,
+ * sect. 2.1-2.3): spectral in y only, real space in x.  PAPER.md:61: the fields are transposed, extended
+ * in y by the 3/2 rule, transformed to real space, multiplied, transformed back, the additional modes are
+ * deleted, the result is transposed, multiplied with a prefactor and added to the right-hand side.
+ * "The nonlinear term needs as input four arrays, the x and y component of the ExB-velocity
+ * and the derivatives of the distribution function with respect to x and y.  Additionally it needs the
+ * already computed right-hand side".
+ *
+ *   per plane p and x:  N(x,y) = vex*dxg + vey*dyg  on the padded real grid Ny = 3*nky0,
+ *                       rhs[x,j,p] += scale * pref[x] * N^(x,j),  j < nky0,  N^ = (1/Ny) sum_y N e^{-i ky y}
+ *
+ * Layout: every array (vex, vey, dxg, dyg, rhs) is complex128 [nx, nky0, planes], x fastest:
+ * offset(x,j,p) = x + nx*(j + nky0*p); x is a real-space point, j the ky index (ky >= 0; ky < 0 implied by
+ * reality; Im of the j = 0 entries is ignored).  pref: nx doubles (the x-dependent prefactor).
+ * All pointers are DEVICE pointers, caller-owned, 16-byte aligned (pref: 8); rhs must not overlap an input.
+ * Supported: nky0 in {8, 16, 32} (Ny = 24, 48, 96); any nx >= 1 (tiles of 32 x points, ragged tail allowed).
+ * Asynchronous on `stream`; one kernel launch per compute.  Errors as for gene_nl_* (gene_nl_last_error).
+ * ===================================================================================================== */
+typedef struct gene_nlx_plan gene_nlx_plan;
+
+/* Returns NULL on failure (unsupported nky0, no device, out of memory). */
+gene_nlx_plan* gene_nlx_create(int nx, int nky0, long long planes);
+
+int gene_nlx_compute(gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
+                     const double* pref, void* rhs, double scale, void* stream);
+
+/* NULL is a no-op.  Synchronises the device. */
+void gene_nlx_destroy(gene_nlx_plan* h);
+
+/* `what`: 0 planes, 1 Ny, 5 algorithmic bytes per plane (6 planes: 5 in, 1 out),
+ * 6 conventional flops per plane (4 c2r + 1 r2c of length Ny per x at 2.5 N log2 N, multiply, prefactor+add). */
+double gene_nlx_query(const gene_nlx_plan* h, int what);
+
 #ifdef __cplusplus
 }
 #endif

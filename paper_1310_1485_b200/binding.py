@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = (
     "gene_nl_create", "gene_nl_compute", "gene_nl_compute_profiled", "gene_nl_compute_host", "gene_nl_destroy",
     "gene_nl_last_error",
     "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query", "gene_nl_probe_peaks",
+    "gene_nlx_create", "gene_nlx_compute", "gene_nlx_destroy", "gene_nlx_query",
 )
 
 _lock = threading.Lock()
@@ -65,6 +66,15 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_query.restype = dbl
         lib.gene_nl_probe_peaks.argtypes = [ctypes.POINTER(dbl)]
         lib.gene_nl_probe_peaks.restype = i
+        ll = ctypes.c_longlong
+        lib.gene_nlx_create.argtypes = [i, i, ll]
+        lib.gene_nlx_create.restype = vp
+        lib.gene_nlx_compute.argtypes = [vp, vp, vp, vp, vp, vp, vp, dbl, vp]
+        lib.gene_nlx_compute.restype = i
+        lib.gene_nlx_destroy.argtypes = [vp]
+        lib.gene_nlx_destroy.restype = None
+        lib.gene_nlx_query.argtypes = [vp, i]
+        lib.gene_nlx_query.restype = dbl
         _lib = lib
         return lib
 
@@ -151,6 +161,36 @@ def gene_nl_probe_peaks():
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_probe_peaks failed ({rc})")
     return float(out[0]), float(out[1]), float(out[2])
+
+
+# ---- x-global variant (include/gene_nl.h, gene_nlx_*) ----
+def gene_nlx_create(nx, nky0, planes) -> int:
+    h = load_library().gene_nlx_create(int(nx), int(nky0), int(planes))
+    if not h:
+        raise GeneNLError(gene_nl_last_error() or "gene_nlx_create failed")
+    return h
+
+
+def gene_nlx_compute(h, vex, vey, dxg, dyg, pref, rhs, scale, stream=None) -> None:
+    """rhs += scale*pref[x]*N^ on DEVICE arrays (torch CUDA tensors or raw addresses); asynchronous on `stream`."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    rc = load_library().gene_nlx_compute(h, _ptr(vex), _ptr(vey), _ptr(dxg), _ptr(dyg), _ptr(pref), _ptr(rhs),
+                                         float(scale), int(stream) or None)
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nlx_compute failed ({rc}): {gene_nl_last_error()}")
+
+
+def gene_nlx_destroy(h) -> None:
+    if h:
+        load_library().gene_nlx_destroy(h)
+
+
+def gene_nlx_query(h, what: int) -> float:
+    return float(load_library().gene_nlx_query(h, int(what)))
 
 
 class GeneNL:

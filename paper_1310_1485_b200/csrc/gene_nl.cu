@@ -422,6 +422,9 @@ extern "C" {
 
 const char* gene_nl_last_error(void) { return g_err.c_str(); }
 
+// internal (not in the header): lets the other translation units of the library set the same thread-local string
+void gene_nl_set_error_(const char* msg) { g_err = msg ? msg : ""; }
+
 gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspec, double kxmin, double kymin,
                              int chi_has_v)
 {

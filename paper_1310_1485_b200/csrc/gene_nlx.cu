@@ -1,0 +1,150 @@
+// gene_nlx.cu -- C ABI of the x-global nonlinearity (include/gene_nl.h, gene_nlx_*): plan, launch.
+// One kernel (nlx_kernel.cuh) per compute; nothing but the twiddle table lives in the plan.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/gene_nl.h"
+#include "nlx_kernel.cuh"
+
+using gnl::cplx;
+
+extern "C" void gene_nl_set_error_(const char* msg);  // gene_nl.cu: the thread-local string of gene_nl_last_error
+
+namespace {
+
+typedef void (*xg_fn)(const cplx*, const cplx*, const cplx*, const cplx*, const double*, cplx*, const cplx*, int, int,
+                      long long, double);
+struct XgKernel {
+    xg_fn fn = nullptr;
+    size_t smem = 0;
+    int nt = 0;
+};
+template <int NY, int A, int B, int NT>
+XgKernel make_xg()
+{
+    XgKernel k;
+    k.fn = gnl::k_xglobal<NY, A, B, NT>;
+    k.smem = gnl::XGlobal<NY, A, B, NT>::SMEM_BYTES;
+    k.nt = NT;
+    return k;
+}
+bool find_xg(int ny, XgKernel* out)
+{
+    switch (ny) {
+    case 24: *out = make_xg<24, 3, 8, 128>(); return true;
+    case 48: *out = make_xg<48, 6, 8, 128>(); return true;   // the paper's 64 x 16 planes
+    case 96: *out = make_xg<96, 12, 8, 128>(); return true;
+    default: return false;
+    }
+}
+
+bool ok_or_err(cudaError_t e, const char* what)
+{
+    if (e == cudaSuccess) return true;
+    gene_nl_set_error_((std::string(what) + ": " + cudaGetErrorString(e)).c_str());
+    return false;
+}
+
+}  // namespace
+
+struct gene_nlx_plan {
+    int nx, nky0, Ny;
+    long long planes;
+    XgKernel k;
+    cplx* tw = nullptr;
+    int grid_cap = 0;
+};
+
+extern "C" {
+
+gene_nlx_plan* gene_nlx_create(int nx, int nky0, long long planes)
+{
+    gene_nl_set_error_("");
+    if (nx <= 0 || nky0 <= 0 || planes <= 0) {
+        gene_nl_set_error_("gene_nlx_create: extents must be positive");
+        return nullptr;
+    }
+    int dev = -1;
+    if (!ok_or_err(cudaGetDevice(&dev), "cudaGetDevice (no CUDA device: this library has no CPU fallback)")) return nullptr;
+    gene_nlx_plan* h = new gene_nlx_plan();
+    h->nx = nx; h->nky0 = nky0; h->Ny = 3 * nky0; h->planes = planes;
+    if (!find_xg(h->Ny, &h->k)) {
+        gene_nl_set_error_("gene_nlx_create: unsupported nky0 (padded y grid Ny = 3 nky0 must be 24, 48 or 96)");
+        delete h;
+        return nullptr;
+    }
+    std::vector<cplx> t(h->Ny);
+    const long double two_pi = 6.283185307179586476925286766559005768L;
+    for (int k = 0; k < h->Ny; ++k) {
+        const long double ang = two_pi * (long double)k / (long double)h->Ny;
+        t[k].x = (double)cosl(ang);
+        t[k].y = (double)sinl(ang);
+    }
+    int sms = 0, occ = 0;
+    bool ok = ok_or_err(cudaMalloc(&h->tw, sizeof(cplx) * h->Ny), "cudaMalloc(twiddles)") &&
+              ok_or_err(cudaMemcpy(h->tw, t.data(), sizeof(cplx) * h->Ny, cudaMemcpyHostToDevice), "cudaMemcpy(twiddles)") &&
+              ok_or_err(cudaFuncSetAttribute(h->k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->k.smem), "k_xglobal smem") &&
+              ok_or_err(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute") &&
+              ok_or_err(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->k.fn, h->k.nt, h->k.smem), "occupancy(k_xglobal)");
+    if (!ok || occ < 1) {
+        if (ok) gene_nl_set_error_("k_xglobal does not fit on an SM");
+        gene_nlx_destroy(h);
+        return nullptr;
+    }
+    h->grid_cap = occ * sms * 8;  // grid-stride over the tiles, a few CTAs per resident slot
+    return h;
+}
+
+int gene_nlx_compute(gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
+                     const double* pref, void* rhs, double scale, void* stream)
+{
+    gene_nl_set_error_("");
+    if (!h) { gene_nl_set_error_("NULL plan"); return GENE_NL_EINVAL; }
+    if (!vex || !vey || !dxg || !dyg || !pref || !rhs) { gene_nl_set_error_("NULL array pointer"); return GENE_NL_EINVAL; }
+    if (((uintptr_t)vex | (uintptr_t)vey | (uintptr_t)dxg | (uintptr_t)dyg | (uintptr_t)rhs) & 15) {
+        gene_nl_set_error_("array pointers must be 16-byte aligned");
+        return GENE_NL_EINVAL;
+    }
+    const size_t bytes = sizeof(cplx) * (size_t)h->nx * h->nky0 * (size_t)h->planes;
+    const char* r0 = (const char*)rhs;
+    for (const void* in : {vex, vey, dxg, dyg}) {
+        const char* a = (const char*)in;
+        if (a < r0 + bytes && r0 < a + bytes) { gene_nl_set_error_("rhs overlaps an input array"); return GENE_NL_EINVAL; }
+    }
+    const int xtiles = (h->nx + 31) / 32;
+    const long long ntiles = h->planes * xtiles;
+    const int grid = (int)(ntiles < h->grid_cap ? ntiles : h->grid_cap);
+    const double coef = scale / (2.0 * (double)h->Ny);
+    h->k.fn<<<grid, h->k.nt, h->k.smem, (cudaStream_t)stream>>>((const cplx*)vex, (const cplx*)vey, (const cplx*)dxg,
+                                                               (const cplx*)dyg, pref, (cplx*)rhs, h->tw, h->nx, xtiles,
+                                                               ntiles, coef);
+    return ok_or_err(cudaGetLastError(), "k_xglobal launch") ? GENE_NL_OK : GENE_NL_ECUDA;
+}
+
+void gene_nlx_destroy(gene_nlx_plan* h)
+{
+    if (!h) return;
+    cudaDeviceSynchronize();
+    cudaFree(h->tw);
+    delete h;
+}
+
+double gene_nlx_query(const gene_nlx_plan* h, int what)
+{
+    if (!h) return NAN;
+    const double M = (double)h->nx * h->nky0, Ny = h->Ny;
+    switch (what) {
+    case 0: return (double)h->planes;
+    case 1: return Ny;
+    case 5: return 16.0 * M * 6.0;  // 5 planes read, 1 written ("5 input, 1 output")
+    case 6: return h->nx * (5.0 * 2.5 * Ny * std::log2(Ny) + 3.0 * Ny) + 4.0 * M;  // 4 c2r + 1 r2c, multiply, prefactor+add
+    default: return NAN;
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,167 @@
+// nlx_kernel.cuh -- the x-GLOBAL E x B nonlinearity, the operator the paper ran and timed:
+// spectral in y only, real space in x.  PAPER.md:61: "the fields are preprocessed (transposition, extension in y
+// direction for dealiasing according to the 3/2-rule) ..., and a fast Fourier transform to real space is applied.
+// After multiplication the result is transformed back to the spectral representation, the additional modes are
+// deleted, the array is transposed and multiplied with a prefactor, and is finally added to the right-hand side
+// vector."  PAPER.md:67: inputs are the x and y components of the E x B velocity and the x and y derivatives of the
+// distribution function, plus the right-hand side (5 planes in, 1 out; intensity 1/6).
+//
+//   per plane, per x:  N(x,y) = vex*dxg + vey*dyg on the padded real grid Ny = 3 nky0,
+//                      rhs[x,j] += scale * pref[x] * N^(x,j),  j < nky0.
+//
+// The paper's seven kernels (Table 3: two transposes, extend, cuFFT x2, multiply, shrink, prefactor) are ONE kernel
+// here, bound by HBM (6 planes of traffic per plane, ~2 flop/B):
+//   * a CTA takes XT = 32 consecutive x of one plane: every global access is a 512 B run along x (the "transposes"
+//     are the index map of the shared-memory staging tile);
+//   * the two real fields of a pair travel as ONE complex field (vex + i vey, dxg + i dyg): one complex y-synthesis
+//     of length Ny gives both; its non-zero inputs are cc in [0,nky0) (+ky) and (2nky0,3nky0) (-ky, conjugates), so
+//     the first radix-A stage is pruned (3/2 rule: "extension" costs no memory and 2/3 of a radix-3 step);
+//   * rows r and r+16 of the tile share ONE forward transform (W = N_r + i N_r+16); the two are separated in the
+//     epilogue, which also deletes the padded modes, applies the prefactor and adds to rhs.
+// Twiddles W_Ny^{jk} come from the global table through L1 (no prologue).  No cuFFT.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "nl_kernels.cuh"
+
+namespace gnl {
+
+template <int NY, int A, int B, int NT>
+struct XGlobal {
+    static constexpr int XT = 32, HP = XT / 2;            // x points (rows) and row pairs per tile
+    static constexpr int NKY0 = NY / 3, W2 = 2 * NKY0;
+    static constexpr int SP = XT + 1;                     // padded row of the staging tile S[field][ky][x]
+    static constexpr int S_CPLX = 4 * NKY0 * SP;
+    static constexpr int FLAT = Tile<A, B>::FLAT;         // exchange tile of one row: [A][BP]
+    static constexpr int E_CPLX = 2 * XT * FLAT;          // (pack, row)
+    static constexpr int PP = W2 + 1;                     // padded row of P[pair][cc] (aliases S)
+    static_assert(HP * PP <= S_CPLX, "P fits over the staging tile");
+    static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)(S_CPLX + E_CPLX);
+};
+
+// grid = planes * ceil(nx / 32); tile t -> plane t / xtiles, x0 = 32 * (t % xtiles)
+template <int NY, int A, int B, int NT>
+__global__ void __launch_bounds__(NT)
+k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx* __restrict__ dxg,
+          const cplx* __restrict__ dyg, const double* __restrict__ pref, cplx* __restrict__ rhs,
+          const cplx* __restrict__ tw_g, int nx, int xtiles, long long ntiles, double coef)
+{
+    using C = XGlobal<NY, A, B, NT>;
+    constexpr int XT = C::XT, HP = C::HP, NKY0 = C::NKY0, W2 = C::W2, SP = C::SP, FLAT = C::FLAT, PP = C::PP;
+    constexpr int A1 = A / 3, BP = Tile<A, B>::BP;
+    extern __shared__ cplx smem[];
+    cplx* S = smem;
+    cplx* E = smem + C::S_CPLX;
+    cplx* Pq = smem;  // over S, once the staging tile has been consumed
+
+    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+        const long long p = t / xtiles;
+        const int x0 = (int)(t % xtiles) * XT;
+        const size_t base = (size_t)p * (size_t)nx * NKY0 + x0;
+
+        // ---- stage the 4 input tiles: S[f][j][r] = F_f[x0 + r + nx j]; lanes over x (transposition = index map) ----
+        for (int item = threadIdx.x; item < 4 * NKY0 * XT; item += NT) {
+            const int r = item % XT, fj = item / XT;
+            const int j = fj % NKY0, f = fj / NKY0;
+            const cplx* F = f == 0 ? vex : f == 1 ? vey : f == 2 ? dxg : dyg;
+            cplx v = cmake(0.0, 0.0);
+            if (x0 + r < nx) v = __ldg(reinterpret_cast<const double2*>(F + base + r + (size_t)nx * j));
+            if (j == 0) v.y = 0.0;  // a real field: Im of the ky = 0 mode is ignored
+            S[fj * SP + r] = v;
+        }
+        __syncthreads();
+
+        // ---- Y1: extension (3/2 rule) + pruned radix-A + twiddle; item = (pack, row, n2) ----
+        for (int item = threadIdx.x; item < 2 * XT * B; item += NT) {
+            const int n2 = item % B, pr = item / B;  // pr = pack * XT + row
+            const int r = pr % XT, pk = pr / XT;
+            const cplx* S1 = S + (2 * pk) * NKY0 * SP + r;   // vex | dxg
+            const cplx* S2 = S1 + NKY0 * SP;                 // vey | dyg
+            cplx lo[A1], hi[A1];
+#pragma unroll
+            for (int a = 0; a < A1; ++a) {
+                const int j = n2 + B * a;                    // +ky: F1 + i F2
+                const cplx f1 = S1[j * SP], f2 = S2[j * SP];
+                lo[a] = cmake(f1.x - f2.y, f1.y + f2.x);
+                const int jm = NKY0 - j;                     // -ky' at cc = j + nky0: conj F1 + i conj F2; ky' = nky0: none
+                const int jc = jm == NKY0 ? 0 : jm;
+                const cplx g1 = S1[jc * SP], g2 = S2[jc * SP];
+                hi[a] = jm == NKY0 ? cmake(0.0, 0.0) : cmake(g1.x + g2.y, g2.x - g1.y);
+            }
+            cplx out[A];
+            dft_pruned_in<A, +1>(lo, hi, out);
+            cplx* Er = E + pr * FLAT + n2;
+#pragma unroll
+            for (int k1 = 0; k1 < A; ++k1) {
+                const cplx w = TWD_G(k1, n2);
+                Er[k1 * BP] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
+            }
+        }
+        __syncthreads();
+
+        // ---- Y2: to real space (both packs, both rows of a pair), multiply, back; item = (pair, k1) ----
+        for (int item = threadIdx.x; item < HP * A; item += NT) {
+            const int k1 = item % A, q = item / A;
+            cplx w[B];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                const int r = q + h * HP;
+                cplx v1[B], v2[B];
+                const cplx* E1 = E + r * FLAT + k1 * BP;
+                const cplx* E2 = E1 + XT * FLAT;
+#pragma unroll
+                for (int n2 = 0; n2 < B; ++n2) { v1[n2] = E1[n2]; v2[n2] = E2[n2]; }
+                Dft<B, +1>::run(v1);  // (vex, vey)(x_r, y = k1 + A k2)
+                Dft<B, +1>::run(v2);  // (dxg, dyg)
+#pragma unroll
+                for (int k2 = 0; k2 < B; ++k2) {
+                    const double nl = fma(v1[k2].x, v2[k2].x, v1[k2].y * v2[k2].y);  // vex dxg + vey dyg
+                    if (h == 0) w[k2].x = nl; else w[k2].y = nl;
+                }
+            }
+            Dft<B, -1>::run(w);
+            cplx* Eo = E + q * FLAT + k1 * BP;  // over the slots this item has just read
+#pragma unroll
+            for (int k2 = 0; k2 < B; ++k2) {
+                const cplx tq = TWD_G(k1, k2);
+                Eo[k2] = (k2 == 0) ? w[0] : cmul(w[k2], tq.x, -tq.y);
+            }
+        }
+        __syncthreads();
+
+        // ---- Y3: pruned-output radix-A ("additional modes are deleted"); item = (pair, k2) -> P[pair][cc] ----
+        for (int item = threadIdx.x; item < HP * B; item += NT) {
+            const int k2 = item % B, q = item / B;
+            cplx in[A];
+            const cplx* Er = E + q * FLAT + k2;
+#pragma unroll
+            for (int n1 = 0; n1 < A; ++n1) in[n1] = Er[n1 * BP];
+            cplx lo[A1], hi[A1];
+            dft_pruned_out<A, -1>(in, lo, hi);
+            cplx* Pr = Pq + q * PP + k2;
+#pragma unroll
+            for (int c = 0; c < A1; ++c) {
+                Pr[B * c] = lo[c];
+                Pr[B * c + NKY0] = hi[c];
+            }
+        }
+        __syncthreads();
+
+        // ---- epilogue: separate the two rows of a pair, prefactor, add to rhs; lanes over x ----
+        for (int item = threadIdx.x; item < NKY0 * XT; item += NT) {
+            const int r = item % XT, j = item / XT;
+            if (x0 + r >= nx) continue;
+            const int q = r % HP;
+            const cplx pp = Pq[q * PP + j], pm = Pq[q * PP + (j ? W2 - j : 0)];
+            // row q: (P+ + conj P-)/2 ; row q + HP: -i (P+ - conj P-)/2   (the 1/2 and 1/Ny are in coef)
+            const cplx n = (r < HP) ? cmake(pp.x + pm.x, pp.y - pm.y) : cmake(pp.y + pm.y, pm.x - pp.x);
+            const double c = coef * __ldg(pref + x0 + r);
+            cplx* R = rhs + base + r + (size_t)nx * j;
+            const cplx o = *R;
+            *R = cmake(fma(c, n.x, o.x), fma(c, n.y, o.y));
+        }
+        __syncthreads();  // P (over S) is free before the next tile is staged
+    }
+}
+
+}  // namespace gnl

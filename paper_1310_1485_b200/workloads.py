@@ -169,3 +169,64 @@ def shard_arrays(wl: Workload, chi, g, rhs, rank: int, world: int):
     rs = rhs.reshape((wl.nw * wl.nspec,) + wl.g_shape[2:])[s0:s1]
     cs = chi.reshape((wl.nw * wl.nspec,) + wl.chi_shape[2:])[s0:s1]
     return sub, cs, gs, rs
+
+
+# ---------------------------------------------------------------------------------------------------------
+# x-global variant: the paper's own workload, 64 x 16 planes ("64 x 16 x 24 x 96
+# x 16" grid points in x, ky, z, v, mu), timed over 589 824 planes device-resident (Table 4).
+# Recipe: five arrays (planes, nky0, nx) complex128, x fastest.  Inputs a+ib ~ N(0,1) with a fall-off 1/(1+(j/4)^2)
+# in the ky index and a smooth envelope in x; the ky = 0 row is real (the fields are real).  rhs ~ N(0,1), ky = 0 row
+# real.  pref[x] = 1 + 0.5*cos(2 pi x/nx) (an x-dependent prefactor), scale = 0.7.  Stands in for GENE data.
+# ---------------------------------------------------------------------------------------------------------
+@dataclass(frozen=True)
+class XGlobalWorkload:
+    name: str
+    nx: int
+    nky0: int
+    planes: int
+    seed: int
+    scale: float
+
+    @property
+    def Ny(self) -> int:
+        return 3 * self.nky0
+
+    @property
+    def shape(self):
+        return (self.planes, self.nky0, self.nx)
+
+    @property
+    def plane_bytes(self) -> int:
+        return 16 * self.nx * self.nky0
+
+
+XGLOBAL_PAPER = XGlobalWorkload("xglobal_paper_64x16_589824", 64, 16, 589824, 6, 0.7)
+XGLOBAL_SMALL = XGlobalWorkload("xglobal_small_64x16_4096", 64, 16, 4096, 7, 0.7)
+
+
+def make_xglobal_inputs(wl: XGlobalWorkload, device="cpu", max_chunk_bytes=1 << 30):
+    """(vex, vey, dxg, dyg, pref, rhs) created on `device` from the workload's seed."""
+    dev = torch.device(device)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(wl.seed)
+    j = torch.arange(wl.nky0, device=dev, dtype=torch.float64)
+    x = torch.arange(wl.nx, device=dev, dtype=torch.float64)
+    damp = (1.0 / (1.0 + (j / 4.0) ** 2))[:, None] * (0.75 + 0.25 * torch.sin(2 * torch.pi * (x + 0.5) / wl.nx))[None, :]
+    step = max(1, max_chunk_bytes // wl.plane_bytes)
+
+    def fill(falloff):
+        out = torch.empty(wl.shape, dtype=torch.complex128, device=dev)
+        for p0 in range(0, wl.planes, step):
+            blk = out[p0:p0 + step]
+            ab = torch.randn(blk.shape + (2,), dtype=torch.float64, device=dev, generator=gen)
+            blk.copy_(torch.view_as_complex(ab))
+            del ab
+            if falloff:
+                blk.mul_(damp)
+            blk[:, 0, :] = blk[:, 0, :].real.to(torch.complex128)
+        return out
+
+    vex, vey, dxg, dyg = (fill(True) for _ in range(4))
+    rhs = fill(False)
+    pref = 1.0 + 0.5 * torch.cos(2 * torch.pi * x / wl.nx)
+    return vex, vey, dxg, dyg, pref, rhs

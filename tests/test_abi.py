@@ -12,12 +12,13 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_functions():
     src = open(os.path.join(ROOT, "include", "gene_nl.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(gene_nl_\w+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(gene_nlx?_\w+)\s*\(", src)))
 
 
 def test_header_declares_the_north_star_entry_points():
     names = declared_functions()
-    for n in ("gene_nl_create", "gene_nl_compute", "gene_nl_destroy"):
+    for n in ("gene_nl_create", "gene_nl_compute", "gene_nl_destroy",
+              "gene_nlx_create", "gene_nlx_compute", "gene_nlx_destroy"):   # x-global variant
         assert n in names
 
 
@@ -47,6 +48,9 @@ def test_no_cpu_fallback_without_a_device():
     from paper_1310_1485_b200 import GeneNLError, gene_nl_create
     with pytest.raises(GeneNLError):
         gene_nl_create(16, 8, 1, 1, 1, 1, 0.1, 0.1, 0)
+    from paper_1310_1485_b200 import gene_nlx_create
+    with pytest.raises(GeneNLError):
+        gene_nlx_create(64, 16, 1)
 
 
 def test_product_path_does_not_touch_the_oracle():
