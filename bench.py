@@ -171,6 +171,152 @@ def reference_arm(args, wl):
     print(json.dumps(line), flush=True)
 
 
+def xglobal_main(args):
+    """`--xglobal`: the x-global variant, the operator and plane shape the paper timed
+    (64 x 16 planes, 589 824 of them device-resident: Table 4).  HBM bound: 6 planes of traffic per
+    plane, so the roofline is bytes / measured HBM bandwidth."""
+    import numpy as np
+    import torch
+
+    from paper_1310_1485_b200 import gene_nlx_compute, gene_nlx_create, gene_nlx_destroy, gene_nlx_query
+    from paper_1310_1485_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    base = W.XGLOBAL_PAPER
+    wl = W.XGlobalWorkload(base.name if args.xglobal_planes == base.planes else f"xglobal_64x16_{args.xglobal_planes}",
+                           base.nx, base.nky0, args.xglobal_planes, base.seed + 1000 * rank, base.scale)
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        import oracle
+        threads = oracle.num_threads()
+        n = 16384
+        sub = W.XGlobalWorkload("sample", wl.nx, wl.nky0, n, wl.seed, wl.scale)
+        a, b, c, d, pref, r = (t.numpy() for t in W.make_xglobal_inputs(sub, "cpu"))
+        for _ in range(args.warmup):
+            oracle.nlx_pseudospectral(a, b, c, d, pref, r, wl.scale)
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            oracle.nlx_pseudospectral(a, b, c, d, pref, r, wl.scale)
+        dt = time.perf_counter() - t0
+        value = n * args.steps / dt
+        sample = f"{n} planes of 64x16 per step, recursive radix-2/3 FFT oracle"
+        print(json.dumps({
+            "impl": "reference", "metric": "x-global ExB nonlinearity planes/s (P_c/s)", "value": value, "unit": UNIT,
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": value / 197e3, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": wl.name, "planes_per_step": n, "nx": wl.nx, "nky0": wl.nky0},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}), flush=True)
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    vex, vey, dxg, dyg, pref, rhs = W.make_xglobal_inputs(wl, dev)
+    h = gene_nlx_create(wl.nx, wl.nky0, wl.planes)
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        gene_nlx_compute(h, vex, vey, dxg, dyg, pref, rhs, wl.scale, stream)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        gene_nlx_compute(h, vex, vey, dxg, dyg, pref, rhs, wl.scale, stream)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_per_step = float(ms.item()) / args.steps
+    value = wl.planes * world / (ms_per_step * 1e-3)
+    B, F = gene_nlx_query(h, 5), gene_nlx_query(h, 6)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    gbs = B * wl.planes / (ms_per_step * 1e-3) / 1e9     # the step IS one launch of k_xglobal
+    traffic = None
+    try:
+        import csv
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
+            if row["workload"] == "xglobal_64x16" and row["kernel"] == "k_xglobal":
+                traffic = float(row["dram_bytes_per_launch"]) * wl.planes / float(row["planes_per_launch"])
+    except Exception:
+        pass
+    roofline = {"kernel": "k_xglobal", "bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
+                "frac": gbs / hbm_peak, "traffic": traffic,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
+                "bytes_per_plane": B, "flops_per_plane": F, "achieved_tflops": F * wl.planes / (ms_per_step * 1e-3) / 1e12,
+                "share_of_step": 1.0}
+    # end to end: pinned host buffers, H2D of the five arrays and D2H of rhs inside the timed region (bounded slice)
+    e2e = None
+    if not args.no_e2e:
+        n = min(wl.planes, 65536)
+        host = [t[:n].cpu().pin_memory() for t in (vex, vey, dxg, dyg, rhs)]
+        devb = [torch.empty_like(t[:n]) for t in (vex, vey, dxg, dyg, rhs)]
+        h2 = gene_nlx_create(wl.nx, wl.nky0, n)
+
+        def once():
+            for hb, db in zip(host, devb):
+                db.copy_(hb, non_blocking=True)
+            gene_nlx_compute(h2, devb[0], devb[1], devb[2], devb[3], pref, devb[4], wl.scale, stream)
+            host[4].copy_(devb[4], non_blocking=True)
+        once()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            once()
+        barrier()
+        dt = time.perf_counter() - t0
+        e2e = {"value": n * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 5 * n * wl.plane_bytes,
+               "d2h_bytes_per_step": n * wl.plane_bytes, "steps": args.e2e_steps,
+               "api": f"torch H2D of 5 arrays + gene_nlx_compute + D2H of rhs on {n} planes (pinned host buffers)"}
+        gene_nlx_destroy(h2)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+        n = 32768
+        sub = W.XGlobalWorkload("sample", wl.nx, wl.nky0, n, wl.seed, wl.scale)
+        a, b, c, d, pr, r = (t.numpy() for t in W.make_xglobal_inputs(sub, "cpu"))
+        t0 = time.perf_counter()
+        oracle.nlx_pseudospectral(a, b, c, d, pr, r, wl.scale)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"{n} planes of 64x16, {dt:.1f} s wall"}
+    gene_nlx_destroy(h)
+    if rank == 0:
+        print(json.dumps({
+            "metric": "x-global ExB nonlinearity planes/s (P_c/s)", "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": value / 197e3, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "nx": wl.nx, "nky0": wl.nky0, "planes_per_gpu": wl.planes,
+                       "padded_y": wl.Ny, "cache": f"inputs larger than L2 ({6 * wl.planes * wl.plane_bytes / 2**30:.1f} GiB per GPU)",
+                       "baseline": "PAPER.md:98-105 Table 4: 197 kP_c/s on one K20X, device-resident (another machine: context)",
+                       "parallelism": f"planes x{world} (independent problems per GPU)"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": args.steps, "roofline": roofline, "cpu_baseline": cpu}), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -182,8 +328,14 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--xglobal", action="store_true",
+                    help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
+    ap.add_argument("--xglobal-planes", type=int, default=589824, help="planes per GPU (Table 4: 589824)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.xglobal:
+        xglobal_main(args)
+        return
 
     from paper_1310_1485_b200 import workloads as W
     wl = W.CONFIGS[args.config]

@@ -26,6 +26,15 @@
 
 namespace gnl {
 
+// 16-byte asynchronous copy global -> shared (LDGSTS); `ok` false writes zeros instead (ragged x tail)
+__device__ __forceinline__ void cp_async16(cplx* dst_smem, const cplx* src, bool ok)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    const int n = ok ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(d), "l"(src), "r"(n) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 template <int NY, int A, int B, int NT>
 struct XGlobal {
     static constexpr int XT = 32, HP = XT / 2;            // x points (rows) and row pairs per tile
@@ -34,12 +43,15 @@ struct XGlobal {
     static constexpr int S_CPLX = 4 * NKY0 * SP;
     static constexpr int FLAT = Tile<A, B>::FLAT;         // exchange tile of one row: [A][BP]
     static constexpr int E_CPLX = 2 * XT * FLAT;          // (pack, row)
-    static constexpr int PP = W2 + 1;                     // padded row of P[pair][cc] (aliases S)
-    static_assert(HP * PP <= S_CPLX, "P fits over the staging tile");
+    static constexpr int PP = W2 + 1;                     // padded row of P[pair][cc]; P lives over the pack-1 tiles of E
+    static_assert(HP * PP <= XT * FLAT, "P fits over the tiles of the second pack");
+    static_assert(NT % 32 == 0 && (4 * NKY0) % (NT / 32) == 0 && NKY0 % (NT / 32) == 0, "staging / epilogue split over the warps");
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)(S_CPLX + E_CPLX);
 };
 
-// grid = planes * ceil(nx / 32); tile t -> plane t / xtiles, x0 = 32 * (t % xtiles)
+// grid-stride over tiles; tile t -> plane t / xtiles, x0 = 32 * (t % xtiles).  Software pipeline per CTA: the inputs
+// of tile t+1 are copied asynchronously into S (free once Y1 of tile t has consumed it) while Y2, Y3 and the epilogue
+// of tile t run; the rhs values of tile t are requested before Y2 and used after Y3.
 template <int NY, int A, int B, int NT>
 __global__ void __launch_bounds__(NT)
 k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx* __restrict__ dxg,
@@ -48,28 +60,38 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
 {
     using C = XGlobal<NY, A, B, NT>;
     constexpr int XT = C::XT, HP = C::HP, NKY0 = C::NKY0, W2 = C::W2, SP = C::SP, FLAT = C::FLAT, PP = C::PP;
-    constexpr int A1 = A / 3, BP = Tile<A, B>::BP;
+    constexpr int A1 = A / 3, BP = Tile<A, B>::BP, NWARP = NT / 32;
+    constexpr int NLD = 4 * NKY0 / NWARP;  // staged (field, ky) rows per warp
+    constexpr int NEP = NKY0 / NWARP;      // epilogue ky rows per warp
     extern __shared__ cplx smem[];
     cplx* S = smem;
     cplx* E = smem + C::S_CPLX;
-    cplx* Pq = smem;  // over S, once the staging tile has been consumed
+    cplx* Pq = E + XT * FLAT;  // over the pack-1 tiles, dead once Y2 has run
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    for (long long t = blockIdx.x; t < ntiles; t += gridDim.x) {
+    // stage the 4 input tiles of tile t: S[f][j][r] = F_f[x0 + r + nx j]; lanes over x (transposition = index map)
+    auto stage = [&](long long t) {
+        const long long p = t / xtiles;
+        const int x0 = (int)(t % xtiles) * XT;
+        const size_t base = (size_t)p * (size_t)nx * NKY0 + x0 + lane;
+        const bool ok = x0 + lane < nx;
+#pragma unroll
+        for (int i = 0; i < NLD; ++i) {
+            const int fj = warp + NWARP * i;       // = f * NKY0 + j
+            const int f = fj / NKY0, j = fj % NKY0;
+            const cplx* F = f == 0 ? vex : f == 1 ? vey : f == 2 ? dxg : dyg;
+            cp_async16(S + fj * SP + lane, ok ? F + base + (size_t)nx * j : F, ok);
+        }
+    };
+
+    long long t = blockIdx.x;
+    if (t < ntiles) stage(t);
+    for (; t < ntiles; t += gridDim.x) {
         const long long p = t / xtiles;
         const int x0 = (int)(t % xtiles) * XT;
         const size_t base = (size_t)p * (size_t)nx * NKY0 + x0;
-
-        // ---- stage the 4 input tiles: S[f][j][r] = F_f[x0 + r + nx j]; lanes over x (transposition = index map) ----
-        for (int item = threadIdx.x; item < 4 * NKY0 * XT; item += NT) {
-            const int r = item % XT, fj = item / XT;
-            const int j = fj % NKY0, f = fj / NKY0;
-            const cplx* F = f == 0 ? vex : f == 1 ? vey : f == 2 ? dxg : dyg;
-            cplx v = cmake(0.0, 0.0);
-            if (x0 + r < nx) v = __ldg(reinterpret_cast<const double2*>(F + base + r + (size_t)nx * j));
-            if (j == 0) v.y = 0.0;  // a real field: Im of the ky = 0 mode is ignored
-            S[fj * SP + r] = v;
-        }
-        __syncthreads();
+        cp_async_wait_all();
+        __syncthreads();  // S holds tile t; everybody is done with E / P of the previous tile
 
         // ---- Y1: extension (3/2 rule) + pruned radix-A + twiddle; item = (pack, row, n2) ----
         for (int item = threadIdx.x; item < 2 * XT * B; item += NT) {
@@ -81,7 +103,8 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
 #pragma unroll
             for (int a = 0; a < A1; ++a) {
                 const int j = n2 + B * a;                    // +ky: F1 + i F2
-                const cplx f1 = S1[j * SP], f2 = S2[j * SP];
+                cplx f1 = S1[j * SP], f2 = S2[j * SP];
+                if (j == 0) { f1.y = 0.0; f2.y = 0.0; }      // real fields: Im of the ky = 0 mode is ignored
                 lo[a] = cmake(f1.x - f2.y, f1.y + f2.x);
                 const int jm = NKY0 - j;                     // -ky' at cc = j + nky0: conj F1 + i conj F2; ky' = nky0: none
                 const int jc = jm == NKY0 ? 0 : jm;
@@ -98,6 +121,15 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
             }
         }
         __syncthreads();
+
+        // S is free: start copying the next tile; request this tile's rhs values (used after Y3)
+        if (t + gridDim.x < ntiles) stage(t + gridDim.x);
+        cplx rv[NEP];
+        const bool okx = x0 + lane < nx;
+#pragma unroll
+        for (int i = 0; i < NEP; ++i)
+            rv[i] = okx ? rhs[base + lane + (size_t)nx * (warp + NWARP * i)] : cmake(0.0, 0.0);
+        const double cpre = okx ? coef * __ldg(pref + x0 + lane) : 0.0;
 
         // ---- Y2: to real space (both packs, both rows of a pair), multiply, back; item = (pair, k1) ----
         for (int item = threadIdx.x; item < HP * A; item += NT) {
@@ -148,19 +180,17 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
         __syncthreads();
 
         // ---- epilogue: separate the two rows of a pair, prefactor, add to rhs; lanes over x ----
-        for (int item = threadIdx.x; item < NKY0 * XT; item += NT) {
-            const int r = item % XT, j = item / XT;
-            if (x0 + r >= nx) continue;
-            const int q = r % HP;
-            const cplx pp = Pq[q * PP + j], pm = Pq[q * PP + (j ? W2 - j : 0)];
-            // row q: (P+ + conj P-)/2 ; row q + HP: -i (P+ - conj P-)/2   (the 1/2 and 1/Ny are in coef)
-            const cplx n = (r < HP) ? cmake(pp.x + pm.x, pp.y - pm.y) : cmake(pp.y + pm.y, pm.x - pp.x);
-            const double c = coef * __ldg(pref + x0 + r);
-            cplx* R = rhs + base + r + (size_t)nx * j;
-            const cplx o = *R;
-            *R = cmake(fma(c, n.x, o.x), fma(c, n.y, o.y));
+        if (okx) {
+            const int q = lane % HP;
+#pragma unroll
+            for (int i = 0; i < NEP; ++i) {
+                const int j = warp + NWARP * i;
+                const cplx pp = Pq[q * PP + j], pm = Pq[q * PP + (j ? W2 - j : 0)];
+                // row q: (P+ + conj P-)/2 ; row q + HP: -i (P+ - conj P-)/2   (the 1/2 and 1/Ny are in coef)
+                const cplx n = (lane < HP) ? cmake(pp.x + pm.x, pp.y - pm.y) : cmake(pp.y + pm.y, pm.x - pp.x);
+                rhs[base + lane + (size_t)nx * j] = cmake(fma(cpre, n.x, rv[i].x), fma(cpre, n.y, rv[i].y));
+            }
         }
-        __syncthreads();  // P (over S) is free before the next tile is staged
     }
 }
 
