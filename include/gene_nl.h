@@ -71,6 +71,21 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, 
                     void* stream);
 
 /*
+ * gene_nl_compute_em -- electromagnetic case with chi composed ON THE DEVICE (BASELINE.json
+ * configs[4]: "phi - v_par*A_par is supplied per plane"; "moving more computation to the GPU, while
+ * keeping the amount of transfer constant").  For a plan created with chi_has_v = GENE_NL_CHI_EM:
+ *     rhs[.,.,p] += scale * N(chi_p, g_p),   chi_p = phi_bar[z,w,s] - vpar[v + nv*s] * apar_bar[z,w,s],  p = (z,v,w,s).
+ * phi, apar: DEVICE arrays, complex128 [nx0, nky0, nz, nw, nspec] (the layout of chi without v); vpar: HOST array of
+ * nv*nspec doubles (copied on `stream`; it may be reused by the caller when the call returns).  By linearity the two
+ * fields are transformed to real space once per (z,w,s) and combined inside the bracket kernel, so the per-plane chi
+ * array (as large as g) is never formed, read or transformed.  Other arguments, errors and asynchrony as
+ * gene_nl_compute.  Always the batched kernels.  gene_nl_compute / gene_nl_compute_host reject such a plan.
+ */
+#define GENE_NL_CHI_EM 2
+int gene_nl_compute_em(gene_nl_plan* h, const void* phi, const void* apar, const double* vpar_host, const void* g,
+                       void* rhs, double scale, void* stream);
+
+/*
  * gene_nl_compute_profiled -- gene_nl_compute with a CUDA-event pair recorded on `stream` around every
  * kernel launch, then a stream synchronise.  ms[c] receives the summed device time [ms] and
  * launches[c] the launch count of kernel class c (arrays of GENE_NL_KERNEL_CLASSES entries):

@@ -17,7 +17,8 @@ GENE_NL_OK, GENE_NL_EINVAL, GENE_NL_EUNSUPPORTED, GENE_NL_ECUDA, GENE_NL_ENOMEM 
 
 # every symbol include/gene_nl.h declares
 EXPORTED_SYMBOLS = (
-    "gene_nl_create", "gene_nl_compute", "gene_nl_compute_profiled", "gene_nl_compute_host", "gene_nl_destroy",
+    "gene_nl_create", "gene_nl_compute", "gene_nl_compute_em", "gene_nl_compute_profiled", "gene_nl_compute_host",
+    "gene_nl_destroy",
     "gene_nl_last_error",
     "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query", "gene_nl_probe_peaks",
     "gene_nlx_create", "gene_nlx_compute", "gene_nlx_destroy", "gene_nlx_query",
@@ -50,6 +51,8 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_create.restype = vp
         lib.gene_nl_compute.argtypes = [vp, vp, vp, vp, dbl, vp]
         lib.gene_nl_compute.restype = i
+        lib.gene_nl_compute_em.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp, vp, dbl, vp]
+        lib.gene_nl_compute_em.restype = i
         lib.gene_nl_compute_profiled.argtypes = [vp, vp, vp, vp, dbl, vp, ctypes.POINTER(dbl), ctypes.POINTER(i)]
         lib.gene_nl_compute_profiled.restype = i
         lib.gene_nl_compute_host.argtypes = [vp, vp, vp, vp, dbl]
@@ -86,7 +89,7 @@ def gene_nl_last_error() -> str:
 def gene_nl_create(nx0, nky0, nz, nv, nw, nspec, kxmin, kymin, chi_has_v) -> int:
     """Returns the opaque plan handle (an integer address); raises GeneNLError on failure."""
     h = load_library().gene_nl_create(int(nx0), int(nky0), int(nz), int(nv), int(nw), int(nspec),
-                                      float(kxmin), float(kymin), int(bool(chi_has_v)))
+                                      float(kxmin), float(kymin), int(chi_has_v))  # 0, 1 or GENE_NL_CHI_EM
     if not h:
         raise GeneNLError(gene_nl_last_error() or "gene_nl_create failed")
     return h
@@ -109,6 +112,24 @@ def gene_nl_compute(h, chi, g, rhs, scale, stream=None) -> None:
     rc = load_library().gene_nl_compute(h, _ptr(chi), _ptr(g), _ptr(rhs), float(scale), int(stream) or None)
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_compute failed ({rc}): {gene_nl_last_error()}")
+
+
+GENE_NL_CHI_EM = 2
+
+
+def gene_nl_compute_em(h, phi, apar, vpar, g, rhs, scale, stream=None) -> None:
+    """rhs += scale*N(phi - vpar*apar, g) with chi composed on the device; vpar: nv*nspec floats (host)."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    vals = [float(x) for x in vpar]
+    arr = (ctypes.c_double * len(vals))(*vals)
+    rc = load_library().gene_nl_compute_em(h, _ptr(phi), _ptr(apar), arr, _ptr(g), _ptr(rhs), float(scale),
+                                           int(stream) or None)
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_compute_em failed ({rc}): {gene_nl_last_error()}")
 
 
 KERNEL_CLASSES = ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd", "k_plane_fused")

@@ -41,7 +41,7 @@ struct XGeom { const cplx* src; cplx* Z; int nky0, nzb; long long vstride; doubl
 typedef void (*xinv_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double, double);
 typedef void (*xfwd_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double);
 typedef void (*yreal_fn)(const cplx*, cplx*, const cplx*, int);
-typedef void (*ybr_fn)(const cplx*, const cplx*, cplx*, const cplx*, int, int, int, int);
+typedef void (*ybr_fn)(const cplx*, const cplx*, cplx*, const cplx*, int, int, int, int, const cplx*, const double*);
 typedef void (*fused_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, int, double, double,
                          double);
 
@@ -113,6 +113,7 @@ struct YKernels {
     int ny, rp, rt, nt;
     size_t smem_br, smem_real;
     ybr_fn br;
+    ybr_fn br_em;  // chi = phi_bar - v_par A_par_bar composed in the bracket
     yreal_fn real;
 };
 
@@ -134,7 +135,8 @@ YKernels make_y()
     k.ny = NY; k.rp = RP; k.rt = 2 * RP; k.nt = NT;
     k.smem_br = sizeof(cplx) * (size_t)(2 * RP * gnl::Tile<A, B>::FLAT);  // exchange tiles only (twiddles come through L1)
     k.smem_real = k.smem_br;
-    k.br = gnl::k_ybracket<NY, A, B, RP, NT>;
+    k.br = gnl::k_ybracket<NY, A, B, RP, NT, false>;
+    k.br_em = gnl::k_ybracket<NY, A, B, RP, NT, true>;
     k.real = gnl::k_yreal<NY, A, B, 2 * RP, NT>;
     return k;
 }
@@ -216,6 +218,8 @@ struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
 
 struct gene_nl_plan {
     int nx0, nky0, nz, nv, nw, nspec, chi_has_v;
+    bool em = false;          // created with chi_has_v = 2: phi_bar and A_par_bar are supplied, chi is composed on device
+    double* vp_dev = nullptr; // em: v_par coefficients, nv * nspec
     double kxmin, kymin;
     int Nx, Ny;
     size_t M;       // modes per plane
@@ -310,7 +314,8 @@ bool set_smem(K fn, size_t bytes, const char* name)
 // Enqueue one chunk: planes (zi in [0,nzc), vi in [0,nv)), plane offset zi + vstride*vi from g/rhs;
 // chi planes zi (+ cvstride*vi if chi_has_v) from chi.  Returns number of launches or -1.
 int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long cvstride, const cplx* g,
-                  cplx* rhs, long long vstride, int nzc, double scale, cudaStream_t st, Profiler* prof = nullptr)
+                  cplx* rhs, long long vstride, int nzc, double scale, cudaStream_t st, Profiler* prof = nullptr,
+                  const cplx* apar = nullptr, const double* vp = nullptr)
 {
     const XKernels& xk = h->xk;
     const YKernels& yk = h->yk;
@@ -326,6 +331,13 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
         GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx)));
         launches += 2;
     }
+    cplx* R2 = nullptr;
+    if (apar) {  // em: the same two kernels on A_par_bar; its real-space fields follow those of phi_bar in R
+        R2 = s.R + (size_t)h->nzb * h->Nx * h->Ny;
+        GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nzc * xt, xk.nt, xk.smem_inv, st>>>(apar, s.Z, h->twx, h->nky0, nzc, 0, h->kxmin, h->kymin)));
+        GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, R2, h->twy, h->Nx)));
+        launches += 2;
+    }
     for (int v0 = 0; v0 < h->nv; v0 += h->nvb) {
         const int nvc = (h->nv - v0 < h->nvb) ? h->nv - v0 : h->nvb;
         const int nb = nzc * nvc;
@@ -337,7 +349,10 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
             launches += 2;
         }
         GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin)));
-        GNL_LAUNCH(prof, K_YBRACKET, (yk.br<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, h->chi_has_v, vfast)));
+        if (apar)
+            GNL_LAUNCH(prof, K_YBRACKET, (yk.br_em<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, 0, vfast, R2, vp + v0)));
+        else
+            GNL_LAUNCH(prof, K_YBRACKET, (yk.br<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, h->chi_has_v, vfast, nullptr, nullptr)));
         GNL_LAUNCH(prof, K_XFWD, (xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef)));
         launches += 3;
     }
@@ -347,7 +362,7 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
 
 // Enqueue `nslab` contiguous (w,s) slabs (standard strides: v stride nz planes).  Returns launches or -1.
 int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx* g, cplx* rhs, int nslab,
-                  double scale, cudaStream_t st, Profiler* prof = nullptr)
+                  double scale, cudaStream_t st, Profiler* prof = nullptr, const cplx* apar = nullptr)
 {
     int launches = 0;
     if (h->fused) {
@@ -394,7 +409,9 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
             const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * sl) * h->M;
             const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * sl) * h->M;
-            int n = enqueue_chunk(h, sc, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, str, prof);
+            // em: slab sl = w + nw * species; its v_par coefficients are vp_dev[nv * species ..]
+            int n = enqueue_chunk(h, sc, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, str, prof,
+                                  apar ? apar + coff : nullptr, apar ? h->vp_dev + (size_t)h->nv * (sl / h->nw) : nullptr);
             if (n < 0) return -1;
             launches += n;
         }
@@ -413,7 +430,7 @@ int chunks_per_slab(const gene_nl_plan* h) { return (h->nz + h->nzb - 1) / h->nz
 int launches_per_chunk(const gene_nl_plan* h)
 {
     const int nbatch = (h->nv + h->nvb - 1) / h->nvb;
-    return h->chi_has_v ? 5 * nbatch : 2 + 3 * nbatch;
+    return h->chi_has_v ? 5 * nbatch : (h->em ? 4 : 2) + 3 * nbatch;
 }
 
 }  // namespace
@@ -438,7 +455,8 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice (no CUDA device: this library has no CPU fallback)")) return nullptr;
     gene_nl_plan* h = new gene_nl_plan();
     h->nx0 = nx0; h->nky0 = nky0; h->nz = nz; h->nv = nv; h->nw = nw; h->nspec = nspec;
-    h->chi_has_v = chi_has_v ? 1 : 0;
+    h->em = chi_has_v == GENE_NL_CHI_EM;
+    h->chi_has_v = (chi_has_v && !h->em) ? 1 : 0;
     h->kxmin = kxmin; h->kymin = kymin;
     h->Nx = 3 * nx0 / 2; h->Ny = 3 * nky0;
     h->M = (size_t)nx0 * nky0;
@@ -462,11 +480,11 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     const size_t budget = scratch_budget_bytes();
     int nzb = nz;
     if (!h->chi_has_v) {
-        while (nzb > 1 && (size_t)nzb * rpp > budget / 4) nzb = (nzb + 1) / 2;
+        while (nzb > 1 && (size_t)nzb * rpp * (h->em ? 2 : 1) > budget / 4) nzb = (nzb + 1) / 2;
     }
     const size_t per_plane = zpp + ppp + (h->chi_has_v ? rpp : 0);
     while (nzb > 1 && (size_t)nzb * per_plane > budget / 2) nzb = (nzb + 1) / 2;
-    const size_t fixed = h->chi_has_v ? 0 : (size_t)nzb * rpp;
+    const size_t fixed = h->chi_has_v ? 0 : (size_t)nzb * rpp * (h->em ? 2 : 1);
     long long nvb = (long long)((budget > fixed ? budget - fixed : 0) / ((size_t)nzb * per_plane));
     if (nvb < 1) nvb = 1;
     if (nvb > nv) nvb = nv;
@@ -474,12 +492,12 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     const size_t nb = (size_t)nzb * nvb;
     h->zbytes = zpp * nb;
     h->pbytes = ppp * nb;
-    h->rbytes = rpp * (h->chi_has_v ? nb : (size_t)nzb);
+    h->rbytes = rpp * (h->chi_has_v ? nb : (size_t)nzb * (h->em ? 2 : 1));
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
     {
         const char* e = getenv("GENE_NL_NO_FUSED");  // development knob: force the batched kernels
         const char* e1 = getenv("GENE_NL_FUSED_V1");  // development knob: first-generation fused kernel
-        const bool want = !(e && atoi(e));
+        const bool want = !(e && atoi(e)) && !h->em;  // the composition lives in k_ybracket (batched path)
         h->fused = want && ((!(e1 && atoi(e1)) && find_fused2(h->Nx, h->Ny, &h->fk)) || find_fused(h->Nx, h->Ny, &h->fk));
     }
     if (h->fused) {
@@ -502,6 +520,8 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     }
 
     bool ok = upload_twiddles(h->Nx, &h->twx) && upload_twiddles(h->Ny, &h->twy) && alloc_scratch(h, &h->scr) &&
+              (!h->em || cuda_ok(cudaMalloc(&h->vp_dev, sizeof(double) * (size_t)nv * nspec), "cudaMalloc(v_par)")) &&
+              (!h->em || set_smem(h->yk.br_em, h->yk.smem_br, "k_ybracket(em) smem")) &&
               set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
               set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
               (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
@@ -550,6 +570,7 @@ void gene_nl_destroy(gene_nl_plan* h)
     free_scratch(&h->scr);
     cudaFree(h->twx);
     cudaFree(h->twy);
+    cudaFree(h->vp_dev);
     delete h;
 }
 
@@ -568,6 +589,7 @@ static int compute_impl(gene_nl_plan* h, const void* chi_, const void* g_, void*
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    if (h->em) { set_err("plan was created with GENE_NL_CHI_EM: call gene_nl_compute_em"); return GENE_NL_EINVAL; }
     const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
     const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
     int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
@@ -578,6 +600,28 @@ static int compute_impl(gene_nl_plan* h, const void* chi_, const void* g_, void*
     cudaStream_t st = (cudaStream_t)stream;
     if (prof) prof->st = st;
     if (enqueue_slabs(h, h->scr, chi, g, rhs, h->nw * h->nspec, scale, st, prof) < 0) return GENE_NL_ECUDA;
+    return GENE_NL_OK;
+}
+
+extern "C" int gene_nl_compute_em(gene_nl_plan* h, const void* phi_, const void* apar_, const double* vpar_host,
+                                  const void* g_, void* rhs_, double scale, void* stream)
+{
+    g_err.clear();
+    if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    if (!h->em) { set_err("gene_nl_compute_em needs a plan created with chi_has_v = GENE_NL_CHI_EM"); return GENE_NL_EINVAL; }
+    if (!vpar_host) { set_err("NULL v_par array"); return GENE_NL_EINVAL; }
+    const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
+    const size_t cbytes = gbytes / h->nv;
+    int rc = check_ptrs(phi_, g_, rhs_, gbytes, cbytes);
+    if (!rc) rc = check_ptrs(apar_, g_, rhs_, gbytes, cbytes);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!cuda_ok(cudaMemcpyAsync(h->vp_dev, vpar_host, sizeof(double) * (size_t)h->nv * h->nspec, cudaMemcpyHostToDevice, st),
+                 "cudaMemcpyAsync(v_par)"))
+        return GENE_NL_ECUDA;
+    if (enqueue_slabs(h, h->scr, (const cplx*)phi_, (const cplx*)g_, (cplx*)rhs_, h->nw * h->nspec, scale, st, nullptr,
+                      (const cplx*)apar_) < 0)
+        return GENE_NL_ECUDA;
     return GENE_NL_OK;
 }
 
@@ -611,6 +655,7 @@ int gene_nl_compute_host(gene_nl_plan* h, const void* chi_, const void* g_, void
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    if (h->em) { set_err("gene_nl_compute_host: not available for GENE_NL_CHI_EM plans"); return GENE_NL_EINVAL; }
     const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
     const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
     int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
@@ -673,7 +718,7 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h)
 double gene_nl_query(const gene_nl_plan* h, int what)
 {
     if (!h) return NAN;
-    const double c = h->chi_has_v ? 1.0 : 1.0 / h->nv;
+    const double c = h->chi_has_v ? 1.0 : (h->em ? 2.0 : 1.0) / h->nv;  // em: two chi-like fields per (z,w,s)
     const double M = (double)h->M, Nx = h->Nx, Ny = h->Ny;
     switch (what) {
     case 0: return (double)h->planes;
@@ -686,7 +731,7 @@ double gene_nl_query(const gene_nl_plan* h, int what)
     case 5: return 16.0 * M * (3.0 + c);
     case 6: {
         const double t2d = h->nky0 * 5.0 * Nx * std::log2(Nx) + Nx * 2.5 * Ny * std::log2(Ny);
-        return (3.0 + 2.0 * c) * t2d + 4.0 * M * (1.0 + c) + 3.0 * Nx * Ny + 4.0 * M;
+        return (3.0 + 2.0 * c) * t2d + 4.0 * M * (1.0 + c) + (h->em ? 7.0 : 3.0) * Nx * Ny + 4.0 * M;  // em: +2 FMA/point
     }
     default: return NAN;
     }

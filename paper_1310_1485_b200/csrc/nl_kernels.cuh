@@ -201,10 +201,14 @@ k_yreal(const cplx* __restrict__ Z, cplx* __restrict__ R, const cplx* __restrict
 // k_ybracket: Z[bl][m][cc] (g) and R[ql][m][y] (chi) -> P[bl][pair][cc].
 // grid = planes_in_batch * (Nx/2 / RP); one CTA does RP row pairs (m, m + Nx/2).
 // ------------------------------------------------------------------------------------------------
-template <int NY, int A, int B, int RP, int NT>
+// EM: chi = phi_bar - v_par * A_par_bar is composed HERE, in real space and by linearity:
+// R holds the real-space fields of phi_bar, R2 those of A_par_bar (one plane per z each, shared by all v), and
+// vp[bl / nzb] is the v_par coefficient of plane bl.  Per-plane chi is then never stored nor transformed.
+template <int NY, int A, int B, int RP, int NT, bool EM = false>
 __global__ void __launch_bounds__(NT)
 k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restrict__ P,
-           const cplx* __restrict__ tw_g, int Nx, int nzb, int chi_per_plane, int vfast)
+           const cplx* __restrict__ tw_g, int Nx, int nzb, int chi_per_plane, int vfast,
+           const cplx* __restrict__ R2 = nullptr, const double* __restrict__ vp = nullptr)
 {
     constexpr int A1 = A / 3, NKY0 = NY / 3, W2 = 2 * NKY0;
     constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
@@ -247,9 +251,15 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
             for (int n2 = 0; n2 < B; ++n2) v[n2] = Er[n2];
             Dft<B, +1>::run(v);  // v[k2] = (dx g + i dy g)(m, y = k1 + A*k2)
             const cplx* Rc = R + ((size_t)ql * Nx + m) * NY + k1;
+            [[maybe_unused]] const cplx* Rc2 = EM ? R2 + ((size_t)ql * Nx + m) * NY + k1 : nullptr;
+            [[maybe_unused]] const double vpar = EM ? __ldg(vp + bl / nzb) : 0.0;
 #pragma unroll
             for (int k2 = 0; k2 < B; ++k2) {
-                const cplx c = Rc[A * k2];  // (dx chi, dy chi)
+                cplx c = Rc[A * k2];  // (dx chi, dy chi)
+                if constexpr (EM) {
+                    const cplx a2 = Rc2[A * k2];  // (dx A_par, dy A_par)
+                    c = cmake(fma(-vpar, a2.x, c.x), fma(-vpar, a2.y, c.y));
+                }
                 const double nl = fma(c.x, v[k2].y, -c.y * v[k2].x);  // dx chi dy g - dy chi dx g
                 if (h == 0) w[k2].x = nl; else w[k2].y = nl;
             }

@@ -1,0 +1,101 @@
+"""Electromagnetic case with chi composed on the device (gene_nl_compute_em): parity against
+the CPU oracle fed with chi_p = phi_bar - vpar * apar_bar composed per plane in numpy (FP64), and agreement with the
+per-plane-chi path of the library (chi_has_v = 1) on the same data."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from helpers import TOL, plane_errors
+from paper_1310_1485_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def em_inputs(wl, device):
+    """phi_bar, apar_bar (chi layout without v), vpar (nv*nspec), g, rhs from the workload's seeded generator."""
+    assert not wl.chi_has_v
+    phi, g, rhs = W.make_inputs(wl, device)
+    wl2 = W.Workload(wl.name + "_apar", wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, False,
+                     wl.seed + 77, wl.rhs_random, wl.scale)
+    apar, _, _ = W.make_inputs(wl2, device)
+    v = np.linspace(-3.0, 3.0, wl.nv)
+    vpar = np.concatenate([v * (1.0 + 0.5 * s) for s in range(wl.nspec)])   # species-dependent thermal velocity
+    return phi, apar, vpar, g, rhs
+
+
+def composed_chi(wl, phi, apar, vpar):
+    """(planes, nky0, nx0) numpy: chi_p = phi_q - vpar[v + nv s] apar_q, p = z + nz (v + nv (w + nw s))."""
+    X, A = (W.as_planes(t, wl).cpu().numpy() for t in (phi, apar))
+    chi = np.empty((wl.planes, wl.nky0, wl.nx0), complex)
+    for p in range(wl.planes):
+        z, v = p % wl.nz, (p // wl.nz) % wl.nv
+        ws = p // (wl.nz * wl.nv)
+        s = ws // wl.nw
+        q = z + wl.nz * ws
+        chi[p] = X[q] - vpar[v + wl.nv * s] * A[q]
+    return chi
+
+
+def run_em(wl, phi, apar, vpar, g, rhs):
+    from paper_1310_1485_b200 import GENE_NL_CHI_EM, gene_nl_compute_em, gene_nl_create, gene_nl_destroy
+    out = rhs.clone()
+    h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
+    try:
+        gene_nl_compute_em(h, phi, apar, vpar, g, out, wl.scale)
+        torch.cuda.synchronize()
+    finally:
+        gene_nl_destroy(h)
+    return out
+
+
+SHAPES = [(16, 8, 3, 5, 2, 2), (64, 32, 2, 3, 2, 1), (96, 48, 2, 4, 1, 2), (128, 32, 3, 3, 1, 1), (256, 64, 2, 2, 1, 2),
+          (32, 128, 1, 3, 1, 1)]
+
+
+@pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec", SHAPES)
+def test_em_matches_oracle_on_composed_chi(cuda_device, nx0, nky0, nz, nv, nw, nspec):
+    wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, False, seed=200 + nx0 + nky0)
+    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+    out = run_em(wl, phi, apar, vpar, g, rhs)
+    chi = composed_chi(wl, phi, apar, vpar)
+    G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
+    ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
+    assert plane_errors(wl, W.as_planes(out, wl).cpu().numpy(), ref, R).max() <= TOL
+
+
+def test_em_under_a_tiny_scratch_budget_and_against_the_per_plane_chi_path(cuda_device, monkeypatch):
+    from helpers import gpu_compute
+    monkeypatch.setenv("GENE_NL_SCRATCH_MB", "2")
+    wl = W.small_workload(64, 32, 5, 7, 2, 2, 0.05, 0.05, False, seed=31)
+    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+    out = run_em(wl, phi, apar, vpar, g, rhs)
+    chi = composed_chi(wl, phi, apar, vpar)
+    G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
+    ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
+    assert plane_errors(wl, W.as_planes(out, wl).cpu().numpy(), ref, R).max() <= TOL
+    # the library's own per-plane-chi path on the composed chi
+    wlv = W.small_workload(64, 32, 5, 7, 2, 2, 0.05, 0.05, True, seed=31)
+    chi_t = torch.from_numpy(chi).to(cuda_device).view(wlv.chi_shape)
+    out_v = gpu_compute(wlv, chi_t, g, rhs)
+    d = (out - out_v).abs().max().item()
+    assert d <= 1e-12 * (out_v - rhs).abs().max().item()
+
+
+def test_em_errors(cuda_device):
+    from paper_1310_1485_b200 import (GENE_NL_CHI_EM, GeneNLError, gene_nl_compute, gene_nl_compute_em, gene_nl_create,
+                                      gene_nl_destroy)
+    wl = W.small_workload(32, 16, 2, 2, 1, 1, 0.1, 0.1, False, seed=8)
+    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+    h_em = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
+    h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, 0)
+    try:
+        with pytest.raises(GeneNLError):
+            gene_nl_compute(h_em, phi, g, rhs, 1.0)            # an EM plan takes gene_nl_compute_em only
+        with pytest.raises(GeneNLError):
+            gene_nl_compute_em(h, phi, apar, vpar, g, rhs, 1.0)  # and the reverse
+        with pytest.raises(GeneNLError):
+            gene_nl_compute_em(h_em, phi, apar, vpar, g, g, 1.0)  # rhs overlaps g
+    finally:
+        gene_nl_destroy(h_em)
+        gene_nl_destroy(h)
