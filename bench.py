@@ -317,6 +317,106 @@ def xglobal_main(args):
         dist.destroy_process_group()
 
 
+def em_main(args):
+    """`--em`: configs[args.config]'s grid with chi composed on the device from phi_bar and A_par_bar
+    (gene_nl_compute_em).  Same metric; the per-plane chi array is never formed."""
+    import numpy as np
+    import torch
+
+    from paper_1310_1485_b200 import (GENE_NL_CHI_EM, gene_nl_compute_em, gene_nl_create, gene_nl_destroy,
+                                      gene_nl_launches_per_compute, gene_nl_query)
+    from paper_1310_1485_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    c = W.CONFIGS[args.config]
+    wl = W.Workload(c.name + "_em_composed", c.nx0, c.nky0, c.nz, c.nv, c.nw, c.nspec, c.kxmin, c.kymin, False,
+                    c.seed + 1000 * rank, c.rhs_random, c.scale)
+    wl2 = W.Workload(wl.name + "_apar", c.nx0, c.nky0, c.nz, c.nv, c.nw, c.nspec, c.kxmin, c.kymin, False,
+                     c.seed + 77 + 1000 * rank, c.rhs_random, c.scale)
+    vpar = np.concatenate([np.linspace(-3.0, 3.0, c.nv) * (1.0 + 0.5 * s) for s in range(c.nspec)])
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    phi, g, rhs = W.make_inputs(wl, dev)
+    apar, _, _ = W.make_inputs(wl2, dev)
+    del _
+    h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
+    stream = torch.cuda.current_stream()
+    for _ in range(max(args.warmup, 3)):
+        gene_nl_compute_em(h, phi, apar, vpar, g, rhs, wl.scale, stream)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        gene_nl_compute_em(h, phi, apar, vpar, g, rhs, wl.scale, stream)
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_per_step = float(ms.item()) / args.steps
+    value = wl.planes * world / (ms_per_step * 1e-3)
+    F, B = gene_nl_query(h, 6), gene_nl_query(h, 5)
+    fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    tf = F * wl.planes / (ms_per_step * 1e-3) / 1e12
+    roofline = {"kernel": "whole step (k_xinv, k_ybracket<EM>, k_xfwd; chi side 4 launches per chunk)", "bound": "alu",
+                "achieved": tf, "peak": fp64_model, "unit": "TFLOP/s", "frac": tf / fp64_model, "traffic": None,
+                "peak_source": "model 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md sect. 7)",
+                "flops_per_plane": F, "bytes_per_plane": B}
+    e2e = None
+    if not args.no_e2e:   # pinned host buffers; H2D of g, rhs, phi, apar and D2H of rhs inside the timed region
+        host = [t.cpu().pin_memory() for t in (phi, apar, g, rhs)]
+
+        def once():
+            phi.copy_(host[0], non_blocking=True)
+            apar.copy_(host[1], non_blocking=True)
+            g.copy_(host[2], non_blocking=True)
+            rhs.copy_(host[3], non_blocking=True)
+            gene_nl_compute_em(h, phi, apar, vpar, g, rhs, wl.scale, stream)
+            host[3].copy_(rhs, non_blocking=True)
+        once()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            once()
+        barrier()
+        dt = time.perf_counter() - t0
+        nb = sum(t.numel() * 16 for t in (phi, apar, g, rhs))
+        e2e = {"value": wl.planes * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": nb,
+               "d2h_bytes_per_step": rhs.numel() * 16, "steps": args.e2e_steps,
+               "api": "torch H2D of phi, apar, g, rhs + gene_nl_compute_em + D2H of rhs (pinned host buffers)"}
+    launches = gene_nl_launches_per_compute(h)
+    gene_nl_destroy(h)
+    if rank == 0:
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": wl.name, "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": wl.planes,
+                       "chi": "composed on device: phi_bar - v_par * A_par_bar (gene_nl_compute_em)",
+                       "cache": "inputs larger than L2", "parallelism": f"planes x{world} (independent problems per GPU)"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches * args.steps, "roofline": roofline,
+            "cpu_baseline": None}), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -330,11 +430,16 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--xglobal", action="store_true",
                     help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
+    ap.add_argument("--em", action="store_true",
+                    help="chi composed on the device from phi_bar and A_par_bar (SURVEY 8(f) f1) on --config's grid")
     ap.add_argument("--xglobal-planes", type=int, default=589824, help="planes per GPU (Table 4: 589824)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.xglobal:
         xglobal_main(args)
+        return
+    if args.em:
+        em_main(args)
         return
 
     from paper_1310_1485_b200 import workloads as W
