@@ -19,6 +19,7 @@
 #include "nl_fused.cuh"
 #include "nl_fused2.cuh"
 #include "nl_kernels.cuh"
+#include "nl_pipe.cuh"
 
 using gnl::cplx;
 
@@ -103,11 +104,15 @@ bool find_fused(int nx, int ny, FusedKernel* out)
     return out->smem <= 227 * 1024;
 }
 
+typedef void (*xinvp_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double, double, int);
 struct XKernels {
     int nx, ck, nt;
     size_t smem_inv, smem_fwd;
     xinv_fn inv;
     xfwd_fn fwd;
+    xinvp_fn invp = nullptr;  // pipelined persistent version (nl_pipe.cuh)
+    size_t smem_invp = 0;
+    int cap_invp = 0;         // its grid (resident CTAs); 0: use the first-generation kernel
 };
 struct YKernels {
     int ny, rp, rt, nt;
@@ -126,6 +131,8 @@ XKernels make_x()
     k.smem_fwd = sizeof(cplx) * (size_t)(A * gnl::Tile<A, B>::BP + CK * gnl::Tile<A, B>::STRIDE);
     k.inv = gnl::k_xinv<NX, A, B, CK, NT>;
     k.fwd = gnl::k_xfwd<NX, A, B, CK, NT>;
+    k.invp = gnl::k_xinv_p<NX, A, B, CK, NT>;
+    k.smem_invp = gnl::XInvP<NX, A, B, CK, NT>::SMEM_BYTES;
     return k;
 }
 template <int NY, int A, int B, int RP, int NT>
@@ -311,6 +318,16 @@ bool set_smem(K fn, size_t bytes, const char* name)
     return cuda_ok(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes), name);
 }
 
+// k_xinv over `ntiles` tiles: the pipelined persistent kernel when enabled, else one CTA per tile
+#define GNL_XINV(prof, st, ntiles, SRC, ZZ, NZB, VSTR)                                                                           \
+    do {                                                                                                                        \
+        if (h->xk.cap_invp > 0)                                                                                                 \
+            GNL_LAUNCH(prof, K_XINV, (h->xk.invp<<<((ntiles) < h->xk.cap_invp ? (ntiles) : h->xk.cap_invp), h->xk.nt, h->xk.smem_invp, st>>>( \
+                                         SRC, ZZ, h->twx, h->nky0, NZB, VSTR, h->kxmin, h->kymin, (ntiles))));                   \
+        else                                                                                                                    \
+            GNL_LAUNCH(prof, K_XINV, (h->xk.inv<<<(ntiles), h->xk.nt, h->xk.smem_inv, st>>>(SRC, ZZ, h->twx, h->nky0, NZB, VSTR, h->kxmin, h->kymin))); \
+    } while (0)
+
 // Enqueue one chunk: planes (zi in [0,nzc), vi in [0,nv)), plane offset zi + vstride*vi from g/rhs;
 // chi planes zi (+ cvstride*vi if chi_has_v) from chi.  Returns number of launches or -1.
 int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long cvstride, const cplx* g,
@@ -327,14 +344,14 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
     // real-space chi of the chunk beyond a third of L2: walk the batch v-fastest (see k_ybracket)
     const int vfast = !h->chi_has_v && (size_t)nzc * h->Nx * h->Ny * sizeof(cplx) > ((size_t)40 << 20);
     if (!h->chi_has_v) {
-        GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nzc * xt, xk.nt, xk.smem_inv, st>>>(chi, s.Z, h->twx, h->nky0, nzc, 0, h->kxmin, h->kymin)));
+        GNL_XINV(prof, st, nzc * xt, chi, s.Z, nzc, 0);
         GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx)));
         launches += 2;
     }
     cplx* R2 = nullptr;
     if (apar) {  // em: the same two kernels on A_par_bar; its real-space fields follow those of phi_bar in R
         R2 = s.R + (size_t)h->nzb * h->Nx * h->Ny;
-        GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nzc * xt, xk.nt, xk.smem_inv, st>>>(apar, s.Z, h->twx, h->nky0, nzc, 0, h->kxmin, h->kymin)));
+        GNL_XINV(prof, st, nzc * xt, apar, s.Z, nzc, 0);
         GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nzc * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, R2, h->twy, h->Nx)));
         launches += 2;
     }
@@ -344,11 +361,11 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
         const size_t off = (size_t)v0 * (size_t)vstride * h->M;
         if (h->chi_has_v) {
             const size_t coff = (size_t)v0 * (size_t)cvstride * h->M;
-            GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(chi + coff, s.Z, h->twx, h->nky0, nzc, cvstride, h->kxmin, h->kymin)));
+            GNL_XINV(prof, st, nb * xt, chi + coff, s.Z, nzc, cvstride);
             GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx)));
             launches += 2;
         }
-        GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin)));
+        GNL_XINV(prof, st, nb * xt, g + off, s.Z, nzc, vstride);
         if (apar)
             GNL_LAUNCH(prof, K_YBRACKET, (yk.br_em<<<nb * yt_pairs, yk.nt, yk.smem_br, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, 0, vfast, R2, vp + v0)));
         else
@@ -377,7 +394,7 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const cplx* chi0 = chi + (size_t)s0 * cps * h->M;
             for (size_t q0 = 0; q0 < nchi; q0 += (size_t)h->nbz) {
                 const int nb = (int)((nchi - q0 < (size_t)h->nbz) ? nchi - q0 : (size_t)h->nbz);
-                GNL_LAUNCH(prof, K_XINV, (xk.inv<<<nb * xt, xk.nt, xk.smem_inv, st>>>(chi0 + q0 * h->M, s.Z, h->twx, h->nky0, nb, 0, h->kxmin, h->kymin)));
+                GNL_XINV(prof, st, nb * xt, chi0 + q0 * h->M, s.Z, nb, 0);
                 GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
                 launches += 2;
             }
@@ -527,6 +544,16 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
               (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
                                        : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
               upload_const_twiddles();
+    if (ok) {  // pipelined persistent x kernel (GENE_NL_PIPE=0: first-generation kernel)
+        const char* e = getenv("GENE_NL_PIPE");
+        // measured on B200: faster for Nx <= 192 (configs[4]: k_xinv 12.0 -> 10.2 ms), equal at 384, slower at 768
+        const int want = e ? atoi(e) : (h->Nx <= 192 ? 1 : 0);
+        int sms = 0, occ = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if ((want & 1) && h->xk.smem_invp <= 227 * 1024 && set_smem(h->xk.invp, h->xk.smem_invp, "k_xinv_p smem") &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
+            h->xk.cap_invp = occ * sms;
+    }
     if (ok && !h->fused && nw * nspec > 1) {
         const char* e = getenv("GENE_NL_STREAMS");  // development knob: internal streams of the batched path
         int na = e ? atoi(e) : 1;
