@@ -159,7 +159,7 @@ int gene_nl_probe_peaks(double* out3);
  * offset(x,j,p) = x + nx*(j + nky0*p); x is a real-space point, j the ky index (ky >= 0; ky < 0 implied by
  * reality; Im of the j = 0 entries is ignored).  pref: nx doubles (the x-dependent prefactor).
  * All pointers are DEVICE pointers, caller-owned, 16-byte aligned (pref: 8); rhs must not overlap an input.
- * Supported: nky0 in {8, 16, 32} (Ny = 24, 48, 96); any nx >= 1 (tiles of 32 x points, ragged tail allowed).
+ * Supported: nky0 in {8, 16, 32} (Ny = 24, 48, 96); any nx >= 1 (tiles of 16 x points, ragged tail allowed).
  * Asynchronous on `stream`; one kernel launch per compute.  Errors as for gene_nl_* (gene_nl_last_error).
  * ===================================================================================================== */
 typedef struct gene_nlx_plan gene_nlx_plan;

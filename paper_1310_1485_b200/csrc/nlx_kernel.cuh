@@ -11,12 +11,12 @@
 //
 // The paper's seven kernels (Table 3: two transposes, extend, cuFFT x2, multiply, shrink, prefactor) are ONE kernel
 // here, bound by HBM (6 planes of traffic per plane, ~2 flop/B):
-//   * a CTA takes XT = 32 consecutive x of one plane: every global access is a 512 B run along x (the "transposes"
+//   * a CTA takes XT = 16 consecutive x of one plane: every global access is a 256 B run along x (the "transposes"
 //     are the index map of the shared-memory staging tile);
 //   * the two real fields of a pair travel as ONE complex field (vex + i vey, dxg + i dyg): one complex y-synthesis
 //     of length Ny gives both; its non-zero inputs are cc in [0,nky0) (+ky) and (2nky0,3nky0) (-ky, conjugates), so
 //     the first radix-A stage is pruned (3/2 rule: "extension" costs no memory and 2/3 of a radix-3 step);
-//   * rows r and r+16 of the tile share ONE forward transform (W = N_r + i N_r+16); the two are separated in the
+//   * rows r and r+XT/2 of the tile share ONE forward transform (W = N_r + i N_r'); the two are separated in the
 //     epilogue, which also deletes the padded modes, applies the prefactor and adds to rhs.
 // Twiddles W_Ny^{jk} come from the global table through L1 (no prologue).  No cuFFT.
 #pragma once
@@ -35,9 +35,9 @@ __device__ __forceinline__ void cp_async16(cplx* dst_smem, const cplx* src, bool
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-template <int NY, int A, int B, int NT>
+template <int NY, int A, int B, int NT, int XT_ = 32>
 struct XGlobal {
-    static constexpr int XT = 32, HP = XT / 2;            // x points (rows) and row pairs per tile
+    static constexpr int XT = XT_, HP = XT / 2;           // x points (rows) and row pairs per tile
     static constexpr int NKY0 = NY / 3, W2 = 2 * NKY0;
     static constexpr int SP = XT + 1;                     // padded row of the staging tile S[field][ky][x]
     static constexpr int S_CPLX = 4 * NKY0 * SP;
@@ -45,29 +45,29 @@ struct XGlobal {
     static constexpr int E_CPLX = 2 * XT * FLAT;          // (pack, row)
     static constexpr int PP = W2 + 1;                     // padded row of P[pair][cc]; P lives over the pack-1 tiles of E
     static_assert(HP * PP <= XT * FLAT, "P fits over the tiles of the second pack");
-    static_assert(NT % 32 == 0 && (4 * NKY0) % (NT / 32) == 0 && NKY0 % (NT / 32) == 0, "staging / epilogue split over the warps");
+    static_assert(NT % XT == 0 && (4 * NKY0) % (NT / XT) == 0 && NKY0 % (NT / XT) == 0, "staging / epilogue split over the threads");
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)(S_CPLX + E_CPLX);
 };
 
 // grid-stride over tiles; tile t -> plane t / xtiles, x0 = 32 * (t % xtiles).  Software pipeline per CTA: the inputs
 // of tile t+1 are copied asynchronously into S (free once Y1 of tile t has consumed it) while Y2, Y3 and the epilogue
 // of tile t run; the rhs values of tile t are requested before Y2 and used after Y3.
-template <int NY, int A, int B, int NT>
+template <int NY, int A, int B, int NT, int XT_ = 32>
 __global__ void __launch_bounds__(NT)
 k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx* __restrict__ dxg,
           const cplx* __restrict__ dyg, const double* __restrict__ pref, cplx* __restrict__ rhs,
           const cplx* __restrict__ tw_g, int nx, int xtiles, long long ntiles, double coef)
 {
-    using C = XGlobal<NY, A, B, NT>;
+    using C = XGlobal<NY, A, B, NT, XT_>;
     constexpr int XT = C::XT, HP = C::HP, NKY0 = C::NKY0, W2 = C::W2, SP = C::SP, FLAT = C::FLAT, PP = C::PP;
-    constexpr int A1 = A / 3, BP = Tile<A, B>::BP, NWARP = NT / 32;
+    constexpr int A1 = A / 3, BP = Tile<A, B>::BP, NWARP = NT / XT;  // "warp" = group of XT threads running over x
     constexpr int NLD = 4 * NKY0 / NWARP;  // staged (field, ky) rows per warp
     constexpr int NEP = NKY0 / NWARP;      // epilogue ky rows per warp
     extern __shared__ cplx smem[];
     cplx* S = smem;
     cplx* E = smem + C::S_CPLX;
     cplx* Pq = E + XT * FLAT;  // over the pack-1 tiles, dead once Y2 has run
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x % XT, warp = threadIdx.x / XT;
 
     // stage the 4 input tiles of tile t: S[f][j][r] = F_f[x0 + r + nx j]; lanes over x (transposition = index map)
     auto stage = [&](long long t) {
