@@ -165,3 +165,32 @@ def test_config1_sampled_modes_against_the_definition(cuda_device):
         N = oracle.nl_convolution_modes(X, G, wl.kxmin, wl.kymin, ii, jj)
         d = (W.as_planes(out, wl)[int(p)] - W.as_planes(rhs, wl)[int(p)]).cpu().numpy()[jj, ii]
         assert np.abs(d - wl.scale * N).max() <= 1e-11 * np.abs(N).max()
+
+
+def test_compute_is_capturable_in_a_cuda_graph(cuda_device):
+    """gene_nl_compute only enqueues kernels on the caller's stream (no synchronisation, no allocation): it can be
+    captured into a CUDA graph and replayed; fused and batched paths."""
+    from paper_1310_1485_b200 import GeneNL
+    for wl in (W.small_workload(128, 32, 2, 3, 1, 1, 0.05, 0.05, False, seed=41),     # fused kernel
+               W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, True, seed=42)):     # batched kernels
+        chi, g, rhs = W.make_inputs(wl, cuda_device)
+        expect = gpu_compute(wl, chi, g, rhs)
+        out = rhs.clone()
+        with GeneNL(wl) as nl:
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                nl.compute(chi, g, out.clone())          # warm-up outside capture
+            torch.cuda.current_stream().wait_stream(side)
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                nl.compute(chi, g, out)                   # torch's capture stream is the current stream here
+            assert torch.equal(out, rhs)                  # nothing ran during capture
+            graph.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(out, expect)
+            graph.replay()                                # rhs keeps accumulating: out = rhs + 2 scale N
+            torch.cuda.synchronize()
+            d = (out - rhs) - 2 * (expect - rhs)
+            assert d.abs().max() <= 1e-13 * (expect - rhs).abs().max()
