@@ -157,11 +157,7 @@ bool find_x(int nx, XKernels* out)
     case 144: *out = make_x<144, 12, 12, 8, 128>(); return true;
     case 192: *out = make_x<192, 24, 8, 8, 128>(); return true;
     case 384: *out = make_x<384, 24, 16, 4, 128>(); return true;
-#ifdef GNL_EXP_X768
-    case 768: *out = make_x<768, 24, 32, 4, GNL_EXP_X768>(); return true;
-#else
     case 768: *out = make_x<768, 24, 32, 4, 128>(); return true;
-#endif
     default: return false;
     }
 }
@@ -175,11 +171,7 @@ bool find_y(int ny, int nx, YKernels* out)
     case 96: *out = rp8 ? make_y<96, 12, 8, 8, 64>() : make_y<96, 12, 8, 4, 64>(); return true;
     case 144: *out = rp8 ? make_y<144, 12, 12, 8, 96>() : make_y<144, 12, 12, 4, 96>(); return true;
     case 192: *out = make_y<192, 12, 16, 4, 64>(); return true;
-#ifdef GNL_EXP_Y384
-    case 384: *out = make_y<384, 24, 16, 4, GNL_EXP_Y384>(); return true;
-#else
     case 384: *out = make_y<384, 24, 16, 4, 64>(); return true;
-#endif
     default: return false;
     }
 }
@@ -213,8 +205,6 @@ struct Profiler {
         if (prof) cudaEventRecord(e_, (prof)->st);          \
     } while (0)
 
-constexpr int kMaxAux = 4;
-
 struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
     cudaStream_t stream = nullptr;
     cplx *g = nullptr, *rhs = nullptr, *chi = nullptr;
@@ -244,12 +234,6 @@ struct gene_nl_plan {
     size_t zbytes, pbytes, rbytes;  // per scratch set
     size_t table_bytes;
     std::vector<HostStage> stages;  // lazily created by gene_nl_compute_host
-    // batched path: (w,s) slabs alternate between internal streams (own scratch each) that fork from and join the
-    // caller's stream, so that the memory-bound and the FP64-bound kernels of neighbouring slabs overlap
-    int naux = 0;
-    cudaStream_t aux[kMaxAux] = {};
-    Scratch aux_scr[kMaxAux];
-    cudaEvent_t ev_fork = nullptr, ev_join[kMaxAux] = {};
     int device;
 };
 
@@ -410,18 +394,9 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
         if (!cuda_ok(cudaGetLastError(), "kernel launch")) return -1;
         return launches;
     }
-    // the plan's own scratch set may fan out over the internal streams; staging sets (host driver) and profiled
-    // runs (one event pair per launch on one stream) stay on the caller's stream
-    const bool fan = (&s == &h->scr) && !prof && h->naux > 1 && nslab > 1;
-    if (fan) {
-        if (!cuda_ok(cudaEventRecord(h->ev_fork, st), "cudaEventRecord(fork)")) return -1;
-        for (int a = 0; a < h->naux; ++a)
-            if (!cuda_ok(cudaStreamWaitEvent(h->aux[a], h->ev_fork, 0), "cudaStreamWaitEvent(fork)")) return -1;
-    }
     for (int sl = 0; sl < nslab; ++sl) {
-        const int a = fan ? sl % h->naux : 0;
-        const Scratch& sc = fan ? h->aux_scr[a] : s;
-        cudaStream_t str = fan ? h->aux[a] : st;
+        const Scratch& sc = s;
+        cudaStream_t str = st;
         for (int z0 = 0; z0 < h->nz; z0 += h->nzb) {
             const int nzc = (h->nz - z0 < h->nzb) ? h->nz - z0 : h->nzb;
             const size_t goff = ((size_t)z0 + (size_t)h->nz * h->nv * sl) * h->M;
@@ -431,12 +406,6 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
                                   apar ? apar + coff : nullptr, apar ? h->vp_dev + (size_t)h->nv * (sl / h->nw) : nullptr);
             if (n < 0) return -1;
             launches += n;
-        }
-    }
-    if (fan) {
-        for (int a = 0; a < h->naux; ++a) {
-            if (!cuda_ok(cudaEventRecord(h->ev_join[a], h->aux[a]), "cudaEventRecord(join)")) return -1;
-            if (!cuda_ok(cudaStreamWaitEvent(st, h->ev_join[a], 0), "cudaStreamWaitEvent(join)")) return -1;
         }
     }
     return launches;
@@ -554,22 +523,6 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
             h->xk.cap_invp = occ * sms;
     }
-    if (ok && !h->fused && nw * nspec > 1) {
-        const char* e = getenv("GENE_NL_STREAMS");  // development knob: internal streams of the batched path
-        int na = e ? atoi(e) : 1;
-        if (na > kMaxAux) na = kMaxAux;
-        if (na > nw * nspec) na = nw * nspec;
-        if (na > 1) {
-            ok = cuda_ok(cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming), "cudaEventCreate");
-            h->aux_scr[0] = h->scr;  // stream 0 works in the plan's own set
-            for (int a = 0; ok && a < na; ++a) {
-                ok = cuda_ok(cudaStreamCreateWithFlags(&h->aux[a], cudaStreamNonBlocking), "cudaStreamCreate") &&
-                     cuda_ok(cudaEventCreateWithFlags(&h->ev_join[a], cudaEventDisableTiming), "cudaEventCreate") &&
-                     (a == 0 || alloc_scratch(h, &h->aux_scr[a]));
-                if (ok) h->naux = a + 1;
-            }
-        }
-    }
     if (!ok) {
         std::string keep = g_err;
         gene_nl_destroy(h);
@@ -588,12 +541,6 @@ void gene_nl_destroy(gene_nl_plan* h)
         free_scratch(&s.scr);
         if (s.stream) cudaStreamDestroy(s.stream);
     }
-    for (int a = 0; a < kMaxAux; ++a) {
-        if (a > 0) free_scratch(&h->aux_scr[a]);
-        if (h->aux[a]) cudaStreamDestroy(h->aux[a]);
-        if (h->ev_join[a]) cudaEventDestroy(h->ev_join[a]);
-    }
-    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     free_scratch(&h->scr);
     cudaFree(h->twx);
     cudaFree(h->twy);
@@ -722,8 +669,7 @@ int gene_nl_compute_host(gene_nl_plan* h, const void* chi_, const void* g_, void
 size_t gene_nl_workspace_bytes(const gene_nl_plan* h)
 {
     if (!h) return 0;
-    const size_t sets = h->naux > 1 ? (size_t)h->naux : 1;
-    return sets * (h->zbytes + h->pbytes + h->rbytes) + h->table_bytes;
+    return h->zbytes + h->pbytes + h->rbytes + h->table_bytes;
 }
 
 int gene_nl_launches_per_compute(const gene_nl_plan* h)

@@ -40,11 +40,7 @@ bool find_xg(int ny, XgKernel* out)
     // 16 x points per tile and 64 threads: 5 CTAs per SM at Ny = 48 (measured on B200: 42.6 M planes/s against 37.4
     // with 32 x points and 128 threads)
     case 24: *out = make_xg<24, 3, 8, 64, 16>(); return true;
-#ifdef GNL_EXP_XG
-    case 48: *out = make_xg<48, 6, 8, GNL_EXP_XG, GNL_EXP_XG_XT>(); return true;
-#else
     case 48: *out = make_xg<48, 6, 8, 64, 16>(); return true;   // the paper's 64 x 16 planes
-#endif
     case 96: *out = make_xg<96, 12, 8, 64, 16>(); return true;
     default: return false;
     }

@@ -110,12 +110,8 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
         const cplx* Fc = F + (size_t)kyi * NX0 + n2;
 #pragma unroll
         for (int a = 0; a < AX1; ++a) {
-#ifdef GNL_EXP_NOG
-            f0[a] = cmake(n2 + a, kyi); f1[a] = cmake(kyi, a);
-#else
             f0[a] = ldg_nc_early(Fc + 8 * a);
             f1[a] = ldg_nc_early(Fc + 8 * a + M);
-#endif
         }
         if (kyi == 0) {  // Hermitian part of the ky = 0 column (reading R7)
 #pragma unroll
@@ -201,11 +197,7 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                 for (int h = 0; h < 2; ++h) {
                     const cplx* Rr = Rc + (size_t)(c + AX * pidx2 + h * NPAIR) * NY + k1y;
 #pragma unroll
-#ifdef GNL_EXP_NOCHI
-                    for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = cmake(k2 + h, lane);
-#else
                     for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc_early(Rr + AY * k2);
-#endif
                 }
                 // -- x stage 2: twiddle (warp-uniform) + radix-8, in place; lanes over 32 columns --
                 {
@@ -242,11 +234,7 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                         for (int h = 0; h < 2; ++h) {
                             const cplx* Rr = Rc + (size_t)(c + AX * (2 + pidx2) + h * NPAIR) * NY + k1y;
 #pragma unroll
-#ifdef GNL_EXP_NOCHI
-                            for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = cmake(k2 + h, lane + (size_t)Rr % 3);
-#else
                             for (int k2 = 0; k2 < 8; ++k2) chv[h][k2] = ldg_nc_early(Rr + AY * k2);
-#endif
                         }
                     }
                     {  // Y1: pruned radix-AY, 4 rows x 8 lanes
@@ -350,12 +338,8 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
             const cplx* Rcol = Rb + (size_t)(4 * warp + (lane >> 3)) * NX0 + (lane & 7);
 #pragma unroll
             for (int c = 0; c < AX1; ++c) {
-#ifdef GNL_EXP_NORHS
-                r0[c] = cmake(1, 2); r1[c] = cmake(3, 4);
-#else
                 r0[c] = ldg_early(Rcol + 8 * c);
                 r1[c] = ldg_early(Rcol + 8 * c + M);
-#endif
             }
         }
         __syncthreads();
