@@ -18,7 +18,8 @@
 //     the first radix-A stage is pruned (3/2 rule: "extension" costs no memory and 2/3 of a radix-3 step);
 //   * rows r and r+XT/2 of the tile share ONE forward transform (W = N_r + i N_r'); the two are separated in the
 //     epilogue, which also deletes the padded modes, applies the prefactor and adds to rhs.
-// Twiddles W_Ny^{jk} come from the global table through L1 (no prologue).  No cuFFT.
+// Twiddles: the Y1 ones (fixed n2 per thread) sit in registers for the life of the persistent CTA, the Y2 ones come
+// from the global table through L1 (a shared-memory table measured slower).  No cuFFT.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -84,6 +85,12 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
         }
     };
 
+    // Y1 twiddles W_Ny^{k1 n2}: n2 = item % B is the same for every Y1 item of a thread (NT is a multiple of B)
+    static_assert(NT % B == 0, "a thread keeps its n2 over the Y1 items");
+    cplx tw1[A];
+#pragma unroll
+    for (int k1 = 0; k1 < A; ++k1) tw1[k1] = TWD_G(k1, threadIdx.x % B);
+
     long long t = blockIdx.x;
     if (t < ntiles) stage(t);
     for (; t < ntiles; t += gridDim.x) {
@@ -115,10 +122,7 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
             dft_pruned_in<A, +1>(lo, hi, out);
             cplx* Er = E + pr * FLAT + n2;
 #pragma unroll
-            for (int k1 = 0; k1 < A; ++k1) {
-                const cplx w = TWD_G(k1, n2);
-                Er[k1 * BP] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
-            }
+            for (int k1 = 0; k1 < A; ++k1) Er[k1 * BP] = (k1 == 0) ? out[0] : cmul(out[k1], tw1[k1].x, tw1[k1].y);
         }
         __syncthreads();
 
