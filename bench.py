@@ -122,7 +122,8 @@ def time_oracle(wl, seconds, threads):
         oracle.nl_pseudospectral(X, G[:n], R[:n], wl.scale, wl.kxmin, wl.kymin, ci[:n])
         return n, time.perf_counter() - t0
 
-    n, dt = run(threads)                        # calibration: one plane per thread
+    run(threads)                                # warm-up (thread pool, page faults)
+    n, dt = run(4 * threads)                    # calibration: four planes per thread
     want = int(max(threads, min(sub.planes, n / dt * seconds)))
     want -= want % threads
     n, dt = run(max(want, threads))
