@@ -211,12 +211,11 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
 #pragma unroll
                     for (int grp = 0; grp < W2 / 32; ++grp) {
                         const int cc = 32 * grp + lane;
+                        cplx wx[8];
+                        wx[0] = cmake(1.0, 0.0);
 #pragma unroll
-                        for (int n2 = 1; n2 < 8; ++n2) {
-                            const cplx w = c_tw[OFFX + n2 * c];
-                            vv[grp][n2] = cmul(vv[grp][n2], w.x, w.y);
-                        }
-                        Dft<8, +1>::run(vv[grp]);
+                        for (int n2 = 1; n2 < 8; ++n2) wx[n2] = c_tw[OFFX + n2 * c];
+                        dft8_twiddled<+1>(vv[grp], wx);
                         const double sgn = (32 * grp >= NKY0) ? -1.0 : 1.0;  // -ky columns hold the conjugate
 #pragma unroll
                         for (int k2 = 0; k2 < 8; ++k2)
@@ -264,13 +263,8 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
                         for (int n2 = 0; n2 < 8; ++n2) v0[n2] = tile0[n2];
 #pragma unroll
                         for (int n2 = 0; n2 < 8; ++n2) v1[n2] = tile1[n2];
-#pragma unroll
-                        for (int n2 = 1; n2 < 8; ++n2) {
-                            v0[n2] = cmul(v0[n2], tq[n2].x, tq[n2].y);
-                            v1[n2] = cmul(v1[n2], tq[n2].x, tq[n2].y);
-                        }
-                        Dft<8, +1>::run(v0);
-                        Dft<8, +1>::run(v1);
+                        dft8_twiddled<+1>(v0, tq);
+                        dft8_twiddled<+1>(v1, tq);
                         cplx w[8];
 #pragma unroll
                         for (int k2 = 0; k2 < 8; ++k2) {  // dx chi * dy g - dy chi * dx g for rows m and m + NX/2
