@@ -431,6 +431,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--xglobal", action="store_true",
                     help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
+    ap.add_argument("--strong", action="store_true",
+                    help="with --gpus N > 1: shard ONE problem's (w,s) slabs over the ranks instead of one problem per rank")
     ap.add_argument("--em", action="store_true",
                     help="chi composed on the device from phi_bar and A_par_bar (SURVEY 8(f) f1) on --config's grid")
     ap.add_argument("--xglobal-planes", type=int, default=589824, help="planes per GPU (Table 4: 589824)")
@@ -470,9 +472,16 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # every rank owns an independent problem of the workload's shape (weak scaling)
-    my = W.Workload(wl.name, wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin,
-                    wl.chi_has_v, wl.seed + 1000 * rank, wl.rhs_random, wl.scale)
+    if args.strong and world > 1:
+        # ONE problem of the workload's shape, its (w,s) slabs sharded over the ranks: g, rhs and
+        # chi shard together, no exchange.  Each rank generates its own slabs (same recipe, rank-dependent seed).
+        s0, s1 = W.shard_slabs(wl, rank, world)
+        my = W.Workload(f"{wl.name}_rank{rank}of{world}", wl.nx0, wl.nky0, wl.nz, wl.nv, max(s1 - s0, 1), 1, wl.kxmin,
+                        wl.kymin, wl.chi_has_v, wl.seed + 1000 * rank, wl.rhs_random, wl.scale)
+    else:
+        # every rank owns an independent problem of the workload's shape (weak scaling)
+        my = W.Workload(wl.name, wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin,
+                        wl.chi_has_v, wl.seed + 1000 * rank, wl.rhs_random, wl.scale)
     chi, g, rhs = W.make_inputs(my, dev)
     nl = GeneNL(my)
     stream = torch.cuda.current_stream()
@@ -494,7 +503,13 @@ def main():
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)
     ms_total = float(ms.item())
     ms_per_step = ms_total / args.steps
-    planes_total = my.planes * world
+    strong = args.strong and world > 1
+    if strong:
+        pt = torch.tensor([float(my.planes)], dtype=torch.float64, device=dev)
+        dist.all_reduce(pt, op=dist.ReduceOp.SUM)
+        planes_total = int(pt.item())
+    else:
+        planes_total = my.planes * world
     value = planes_total / (ms_per_step * 1e-3)
 
     # per-kernel device time, live, with CUDA events on the launching stream
@@ -583,13 +598,14 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "strong" if strong else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": wl.name, "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": my.planes,
                        "padded_grid": [wl.Nx, wl.Ny], "chi_has_v": wl.chi_has_v,
                        "cache": "inputs larger than L2 (g+rhs+chi = %.0f MiB per GPU)" %
                                 ((2 * my.planes + my.chi_planes) * my.plane_bytes / 2 ** 20),
-                       "parallelism": f"planes x{world} (independent problems per GPU)"},
+                       "parallelism": (f"one problem, (w,s) slabs sharded over {world} GPUs" if strong else f"planes x{world} (independent problems per GPU)")},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
             "roofline": roofline, "roofline_step": roofline_step, "kernels": kernels,
             "cpu_baseline": cpu_baseline,
