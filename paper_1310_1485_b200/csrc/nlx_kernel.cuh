@@ -18,8 +18,9 @@
 //     the first radix-A stage is pruned (3/2 rule: "extension" costs no memory and 2/3 of a radix-3 step);
 //   * rows r and r+XT/2 of the tile share ONE forward transform (W = N_r + i N_r'); the two are separated in the
 //     epilogue, which also deletes the padded modes, applies the prefactor and adds to rhs.
-// Twiddles: the Y1 ones (fixed n2 per thread) sit in registers for the life of the persistent CTA, the Y2 ones come
-// from the global table through L1 (a shared-memory table measured slower).  No cuFFT.
+// Twiddles: the Y1 ones (fixed n2 per thread) sit in registers for the life of the persistent CTA, and so do the Y2
+// ones when a thread has at most one Y2 item per tile (fixed k1); otherwise they come from the global table through L1
+// (a shared-memory table measured slower).  No cuFFT.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -62,8 +63,7 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
     using C = XGlobal<NY, A, B, NT, XT_>;
     constexpr int XT = C::XT, HP = C::HP, NKY0 = C::NKY0, W2 = C::W2, SP = C::SP, FLAT = C::FLAT, PP = C::PP;
     constexpr int A1 = A / 3, BP = Tile<A, B>::BP, NWARP = NT / XT;  // "warp" = group of XT threads running over x
-    constexpr int NLD = 4 * NKY0 / NWARP;  // staged (field, ky) rows per warp
-    constexpr int NEP = NKY0 / NWARP;      // epilogue ky rows per warp
+    constexpr int NEP = NKY0 / NWARP;      // ky rows per group of XT threads (staging of each field, epilogue)
     extern __shared__ cplx smem[];
     cplx* S = smem;
     cplx* E = smem + C::S_CPLX;
@@ -77,11 +77,13 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
         const size_t base = (size_t)p * (size_t)nx * NKY0 + x0 + lane;
         const bool ok = x0 + lane < nx;
 #pragma unroll
-        for (int i = 0; i < NLD; ++i) {
-            const int fj = warp + NWARP * i;       // = f * NKY0 + j
-            const int f = fj / NKY0, j = fj % NKY0;
+        for (int f = 0; f < 4; ++f) {              // the field is a compile-time index: no pointer selects per copy
             const cplx* F = f == 0 ? vex : f == 1 ? vey : f == 2 ? dxg : dyg;
-            cp_async16(S + fj * SP + lane, ok ? F + base + (size_t)nx * j : F, ok);
+#pragma unroll
+            for (int i = 0; i < NEP; ++i) {
+                const int j = warp + NWARP * i;
+                cp_async16(S + (f * NKY0 + j) * SP + lane, ok ? F + base + (size_t)nx * j : F, ok);
+            }
         }
     };
 
@@ -90,6 +92,14 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
     cplx tw1[A];
 #pragma unroll
     for (int k1 = 0; k1 < A; ++k1) tw1[k1] = TWD_G(k1, threadIdx.x % B);
+
+    // Y2 twiddles W_Ny^{k1 k2}: with at most one Y2 item per thread (HP * A <= NT) k1 = threadIdx.x % A is fixed too
+    constexpr bool TW2_REGS = (HP * A <= NT);
+    [[maybe_unused]] cplx tw2[B];
+    if constexpr (TW2_REGS) {
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) tw2[k2] = TWD_G(threadIdx.x % A, k2);
+    }
 
     long long t = blockIdx.x;
     if (t < ntiles) stage(t);
@@ -159,7 +169,8 @@ k_xglobal(const cplx* __restrict__ vex, const cplx* __restrict__ vey, const cplx
             cplx* Eo = E + q * FLAT + k1 * BP;  // over the slots this item has just read
 #pragma unroll
             for (int k2 = 0; k2 < B; ++k2) {
-                const cplx tq = TWD_G(k1, k2);
+                cplx tq;
+                if constexpr (TW2_REGS) tq = tw2[k2]; else tq = TWD_G(k1, k2);
                 Eo[k2] = (k2 == 0) ? w[0] : cmul(w[k2], tq.x, -tq.y);
             }
         }
