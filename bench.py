@@ -523,6 +523,8 @@ def main():
             prof_ms[k] += m[k]
             prof_n[k] += n[k]
     flops = per_kernel_flops(my, fused=nl.query(7) == 1.0)
+    if my.chi_has_v and not prof_n.get("k_yreal") and "k_yreal" in flops and "k_ybracket" in flops:
+        flops["k_ybracket"] += flops.pop("k_yreal")  # chi's y-synthesis runs inside k_ybracket_cv (no k_yreal launches)
     fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
     try:
         probe_tf, probe_smem_gbs, _ = gene_nl_probe_peaks()

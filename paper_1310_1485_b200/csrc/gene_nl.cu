@@ -114,11 +114,15 @@ struct XKernels {
     size_t smem_invp = 0;
     int cap_invp = 0;         // its grid (resident CTAs); 0: use the first-generation kernel
 };
+typedef void (*ybrcv_fn)(const cplx*, const cplx*, cplx*, const cplx*, int);
 struct YKernels {
     int ny, rp, rt, nt;
     size_t smem_br, smem_real;
     ybr_fn br;
     ybr_fn br_em;  // chi = phi_bar - v_par A_par_bar composed in the bracket
+    ybrcv_fn br_cv;  // chi per plane: its y-synthesis fused into the bracket kernel (no R round trip)
+    size_t smem_cv;
+    int rp_cv;
     yreal_fn real;
 };
 
@@ -144,6 +148,10 @@ YKernels make_y()
     k.smem_real = k.smem_br;
     k.br = gnl::k_ybracket<NY, A, B, RP, NT, false>;
     k.br_em = gnl::k_ybracket<NY, A, B, RP, NT, true>;
+    constexpr int RPC = (RP >= 8) ? RP / 2 : RP;  // twice the exchange tiles per pair: fewer pairs per CTA
+    k.br_cv = gnl::k_ybracket_cv<NY, A, B, RPC, NT>;
+    k.smem_cv = sizeof(cplx) * (size_t)(4 * RPC * gnl::Tile<A, B>::FLAT);
+    k.rp_cv = RPC;
     k.real = gnl::k_yreal<NY, A, B, 2 * RP, NT>;
     return k;
 }
@@ -215,6 +223,7 @@ struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
 
 struct gene_nl_plan {
     int nx0, nky0, nz, nv, nw, nspec, chi_has_v;
+    bool fuse_chi_y = false;  // chi_has_v = 1 on the batched path: chi's y-synthesis inside k_ybracket_cv
     bool em = false;          // created with chi_has_v = 2: phi_bar and A_par_bar are supplied, chi is composed on device
     double* vp_dev = nullptr; // em: v_par coefficients, nv * nspec
     double kxmin, kymin;
@@ -343,6 +352,17 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
         const int nvc = (h->nv - v0 < h->nvb) ? h->nv - v0 : h->nvb;
         const int nb = nzc * nvc;
         const size_t off = (size_t)v0 * (size_t)vstride * h->M;
+        if (h->chi_has_v && h->fuse_chi_y) {
+            // chi per plane: its x-synthesis goes to the R buffer (large enough: Nx*Ny >= Nx*2nky0 per plane) and its
+            // y-synthesis runs inside k_ybracket_cv
+            const size_t coff = (size_t)v0 * (size_t)cvstride * h->M;
+            GNL_XINV(prof, st, nb * xt, chi + coff, s.R, nzc, cvstride);
+            GNL_XINV(prof, st, nb * xt, g + off, s.Z, nzc, vstride);
+            GNL_LAUNCH(prof, K_YBRACKET, (yk.br_cv<<<nb * ((h->Nx / 2) / yk.rp_cv), yk.nt, yk.smem_cv, st>>>(s.Z, s.R, s.P, h->twy, h->Nx)));
+            GNL_LAUNCH(prof, K_XFWD, (xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef)));
+            launches += 4;
+            continue;
+        }
         if (h->chi_has_v) {
             const size_t coff = (size_t)v0 * (size_t)cvstride * h->M;
             GNL_XINV(prof, st, nb * xt, chi + coff, s.Z, nzc, cvstride);
@@ -416,7 +436,7 @@ int chunks_per_slab(const gene_nl_plan* h) { return (h->nz + h->nzb - 1) / h->nz
 int launches_per_chunk(const gene_nl_plan* h)
 {
     const int nbatch = (h->nv + h->nvb - 1) / h->nvb;
-    return h->chi_has_v ? 5 * nbatch : (h->em ? 4 : 2) + 3 * nbatch;
+    return h->chi_has_v ? (h->fuse_chi_y ? 4 : 5) * nbatch : (h->em ? 4 : 2) + 3 * nbatch;
 }
 
 }  // namespace
@@ -522,6 +542,10 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
         if ((want & 1) && h->xk.smem_invp <= 227 * 1024 && set_smem(h->xk.invp, h->xk.smem_invp, "k_xinv_p smem") &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
             h->xk.cap_invp = occ * sms;
+    }
+    if (ok && h->chi_has_v && !h->fused && (h->Nx / 2) % h->yk.rp_cv == 0 && h->yk.smem_cv <= 227 * 1024) {
+        const char* e = getenv("GENE_NL_NO_FUSE_CHI");  // development knob: k_yreal + R round trip instead
+        h->fuse_chi_y = !(e && atoi(e)) && set_smem(h->yk.br_cv, h->yk.smem_cv, "k_ybracket_cv smem");
     }
     if (!ok) {
         std::string keep = g_err;

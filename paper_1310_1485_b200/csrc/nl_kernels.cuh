@@ -293,6 +293,85 @@ k_ybracket(const cplx* __restrict__ Z, const cplx* __restrict__ R, cplx* __restr
 }
 
 // ------------------------------------------------------------------------------------------------
+// k_ybracket_cv: chi per plane (chi_has_v = 1).  Z[bl][m][cc] (g) and Zc[bl][m][cc] (chi, the same x-synthesis) ->
+// P[bl][pair][cc].  With one chi plane per g plane there is nothing to share across v, so the real-space chi
+// fields are NOT written to and read back from HBM (k_yreal + the R reads of k_ybracket: 2 x 4.5 planes of traffic per
+// plane, which made both kernels HBM bound at configs[4]): the y-synthesis of the chi rows runs here, next to that
+// of the g rows.  smem: 4*RP exchange tiles (g rows, then chi rows).  grid = planes_in_batch * (Nx/2 / RP).
+// ------------------------------------------------------------------------------------------------
+template <int NY, int A, int B, int RP, int NT>
+__global__ void __launch_bounds__(NT)
+k_ybracket_cv(const cplx* __restrict__ Z, const cplx* __restrict__ Zc, cplx* __restrict__ P,
+              const cplx* __restrict__ tw_g, int Nx)
+{
+    constexpr int A1 = A / 3, NKY0 = NY / 3, W2 = 2 * NKY0;
+    constexpr int BP = Tile<A, B>::BP, RS = Tile<A, B>::FLAT;
+    extern __shared__ cplx smem[];
+    cplx* E = smem;
+    cplx* Ec = smem + 2 * RP * RS;
+    const int half = Nx / 2;
+    const int ntile = half / RP;
+    const int bl = blockIdx.x / ntile;
+    const int m0 = (blockIdx.x % ntile) * RP;
+
+    // Y1: pruned radix-A + twiddle for the 2*RP rows of g and the 2*RP rows of chi
+    for (int item = threadIdx.x; item < 4 * RP * B; item += NT) {
+        const int n2 = item % B, r4 = item / B;
+        const int r = r4 % (2 * RP), src = r4 / (2 * RP);
+        const int m = m0 + (r % RP) + (r / RP) * half;
+        y_stage1<NY, A, B>((src ? Zc : Z) + ((size_t)bl * Nx + m) * W2, tw_g, E + r4 * RS, n2);
+    }
+    __syncthreads();
+
+    // Y2: both rows of a pair of g and of chi to real space, bracket, radix-B back + twiddle (in place)
+    for (int item = threadIdx.x; item < RP * A; item += NT) {
+        const int k1 = item % A, r = item / A;
+        cplx w[B];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int row = r + h * RP;
+            cplx v[B], c[B];
+            const cplx* Er = E + row * RS + k1 * BP;
+            const cplx* Cr = Ec + row * RS + k1 * BP;
+#pragma unroll
+            for (int n2 = 0; n2 < B; ++n2) { v[n2] = Er[n2]; c[n2] = Cr[n2]; }
+            Dft<B, +1>::run(v);  // (dx g + i dy g)(m, y = k1 + A*k2)
+            Dft<B, +1>::run(c);  // (dx chi + i dy chi)
+#pragma unroll
+            for (int k2 = 0; k2 < B; ++k2) {
+                const double nl = fma(c[k2].x, v[k2].y, -c[k2].y * v[k2].x);  // dx chi dy g - dy chi dx g
+                if (h == 0) w[k2].x = nl; else w[k2].y = nl;
+            }
+        }
+        Dft<B, -1>::run(w);
+        cplx* Er = E + r * RS + k1 * BP;
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) {
+            cplx t = TWD_G(k1, k2);
+            Er[k2] = (k2 == 0) ? w[0] : cmul(w[k2], t.x, -t.y);
+        }
+    }
+    __syncthreads();
+
+    // Y3: pruned-output radix-A over n1 for fixed k2; j = k2 + B*k1
+    for (int item = threadIdx.x; item < RP * B; item += NT) {
+        const int k2 = item % B, r = item / B;
+        cplx in[A];
+        const cplx* Er = E + r * RS + k2;
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) in[n1] = Er[n1 * BP];
+        cplx lo[A1], hi[A1];
+        dft_pruned_out<A, -1>(in, lo, hi);
+        cplx* Pp = P + ((size_t)bl * half + m0 + r) * W2 + k2;
+#pragma unroll
+        for (int c = 0; c < A1; ++c) {
+            Pp[B * c] = lo[c];
+            Pp[B * c + NKY0] = hi[c];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // k_xfwd: P[bl][pair][cc] -> rhs[ky][i] += coef * X.  grid = planes_in_batch * (nky0 / CK).
 // ------------------------------------------------------------------------------------------------
 template <int NX, int A, int B, int CK, int NT>
