@@ -110,16 +110,20 @@ struct XKernels {
     size_t smem_inv, smem_fwd;
     xinv_fn inv;
     xfwd_fn fwd;
+    xinvp_fn invp_zt = nullptr;  // the same, storing Z transposed (for k_ybracket_t)
     xinvp_fn invp = nullptr;  // pipelined persistent version (nl_pipe.cuh)
     size_t smem_invp = 0;
     int cap_invp = 0;         // its grid (resident CTAs); 0: use the first-generation kernel
 };
 typedef void (*ybrcv_fn)(const cplx*, const cplx*, cplx*, const cplx*, int);
+typedef void (*ybrt_fn)(const cplx*, const cplx*, cplx*, const cplx*, int, int, int);
 struct YKernels {
     int ny, rp, rt, nt;
     size_t smem_br, smem_real;
     ybr_fn br;
     ybr_fn br_em;  // chi = phi_bar - v_par A_par_bar composed in the bracket
+    ybrt_fn br_t = nullptr;  // g side read from the transposed Z (tiles of 8 row pairs, 128 threads)
+    size_t smem_t = 0;
     ybrcv_fn br_cv;  // chi per plane: its y-synthesis fused into the bracket kernel (no R round trip)
     size_t smem_cv;
     int rp_cv;
@@ -135,7 +139,8 @@ XKernels make_x()
     k.smem_fwd = sizeof(cplx) * (size_t)(A * gnl::Tile<A, B>::BP + CK * gnl::Tile<A, B>::STRIDE);
     k.inv = gnl::k_xinv<NX, A, B, CK, NT>;
     k.fwd = gnl::k_xfwd<NX, A, B, CK, NT>;
-    k.invp = gnl::k_xinv_p<NX, A, B, CK, NT>;
+    k.invp = gnl::k_xinv_p<NX, A, B, CK, NT, false>;
+    k.invp_zt = gnl::k_xinv_p<NX, A, B, CK, NT, true>;
     k.smem_invp = gnl::XInvP<NX, A, B, CK, NT>::SMEM_BYTES;
     return k;
 }
@@ -148,6 +153,8 @@ YKernels make_y()
     k.smem_real = k.smem_br;
     k.br = gnl::k_ybracket<NY, A, B, RP, NT, false>;
     k.br_em = gnl::k_ybracket<NY, A, B, RP, NT, true>;
+    k.br_t = gnl::k_ybracket_t<NY, A, B, 128, 8>;
+    k.smem_t = gnl::YBracketT<NY, A, B, 128, 8>::SMEM_BYTES;
     constexpr int RPC = (RP >= 8) ? RP / 2 : RP;  // twice the exchange tiles per pair: fewer pairs per CTA
     k.br_cv = gnl::k_ybracket_cv<NY, A, B, RPC, NT>;
     k.smem_cv = sizeof(cplx) * (size_t)(4 * RPC * gnl::Tile<A, B>::FLAT);
@@ -223,6 +230,8 @@ struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
 
 struct gene_nl_plan {
     int nx0, nky0, nz, nv, nw, nspec, chi_has_v;
+    bool zt = false;          // g side through the transposed Z: k_xinv_p<ZT> + k_ybracket_t (chi shared over v only)
+    int cap_invp_zt = 0;
     bool fuse_chi_y = false;  // chi_has_v = 1 on the batched path: chi's y-synthesis inside k_ybracket_cv
     bool em = false;          // created with chi_has_v = 2: phi_bar and A_par_bar are supplied, chi is composed on device
     double* vp_dev = nullptr; // em: v_par coefficients, nv * nspec
@@ -368,6 +377,14 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
             GNL_XINV(prof, st, nb * xt, chi + coff, s.Z, nzc, cvstride);
             GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R, h->twy, h->Nx)));
             launches += 2;
+        }
+        if (h->zt && !apar) {
+            const int ntot = nb * xt;
+            GNL_LAUNCH(prof, K_XINV, (xk.invp_zt<<<(ntot < h->cap_invp_zt ? ntot : h->cap_invp_zt), xk.nt, xk.smem_invp, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin, ntot)));
+            GNL_LAUNCH(prof, K_YBRACKET, (yk.br_t<<<nb * ((h->Nx / 2) / 8), 128, yk.smem_t, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, vfast)));
+            GNL_LAUNCH(prof, K_XFWD, (xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef)));
+            launches += 3;
+            continue;
         }
         GNL_XINV(prof, st, nb * xt, g + off, s.Z, nzc, vstride);
         if (apar)
@@ -542,6 +559,20 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
         if ((want & 1) && h->xk.smem_invp <= 227 * 1024 && set_smem(h->xk.invp, h->xk.smem_invp, "k_xinv_p smem") &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
             h->xk.cap_invp = occ * sms;
+    }
+    if (ok && !h->chi_has_v && !h->em && !h->fused && (h->Nx / 2) % 8 == 0 && h->Ny <= 192 && h->yk.smem_t <= 227 * 1024 &&
+        h->xk.smem_invp <= 227 * 1024) {
+        // measured on B200: 384 x 192 (configs[2]) 7.79 -> 7.19 ms; at Ny = 384 the 105 KB of exchange tiles of
+        // k_ybracket_t cost more than the stores save (configs[3]: 101 -> 119 ms), so that size keeps the row-major Z
+        const char* e = getenv("GENE_NL_ZT");  // development knob
+        int sms = 0, occ = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if ((e ? atoi(e) : 1) && set_smem(h->yk.br_t, h->yk.smem_t, "k_ybracket_t smem") &&
+            set_smem(h->xk.invp_zt, h->xk.smem_invp, "k_xinv_p<ZT> smem") &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp_zt, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0) {
+            h->zt = true;
+            h->cap_invp_zt = occ * sms;
+        }
     }
     if (ok && h->chi_has_v && !h->fused && (h->Nx / 2) % h->yk.rp_cv == 0 && h->yk.smem_cv <= 227 * 1024) {
         const char* e = getenv("GENE_NL_NO_FUSE_CHI");  // development knob: k_yreal + R round trip instead

@@ -30,7 +30,10 @@ struct XInvP {
     static_assert(SG_CPLX % NT == 0, "the staged block splits evenly over the threads");
 };
 
-template <int NX, int A, int B, int CK, int NT>
+// ZT: Z is stored TRANSPOSED, Zt[bl][cc][m]: the 8 consecutive m of a warp's stage-2 items form a 128 B run, where the
+// row-major store scatters 64 B pieces 2 KB apart (measured: the store pattern costs 29 % of the kernel at Nx = 384).
+// k_ybracket_t reads that layout.
+template <int NX, int A, int B, int CK, int NT, bool ZT = false>
 __global__ void __launch_bounds__(NT)
 k_xinv_p(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restrict__ tw_g,
          int nky0, int nzb, long long vstride, double kxmin, double kymin, int ntot)
@@ -124,8 +127,113 @@ k_xinv_p(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restr
 #pragma unroll
             for (int k2 = 0; k2 < B; ++k2) {
                 const int m = k1 + A * k2;
-                Zc[(size_t)m * W2] = sg ? cconj(v[k2]) : v[k2];
+                if constexpr (ZT) Zb[(size_t)cc * NX + m] = sg ? cconj(v[k2]) : v[k2];
+                else Zc[(size_t)m * W2] = sg ? cconj(v[k2]) : v[k2];
             }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------------
+// k_ybracket_t: as k_ybracket (chi shared over v), reading the g side from the TRANSPOSED Zt[bl][cc][m].  A tile is 8
+// row pairs (m0..m0+7 and m0+Nx/2..+7): in Y1 the lanes run over the 16 rows, so every load is two 128 B runs.
+// smem: 16 exchange tiles with an odd row stride (lanes over rows stay bank-conflict free).  grid as k_ybracket, RP = 8.
+// ------------------------------------------------------------------------------------------------------------------
+template <int NY, int A, int B, int NT, int RP_ = 8>
+struct YBracketT {
+    static constexpr int RP = RP_, RSP = odd_up(Tile<A, B>::FLAT);
+    static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)(2 * RP * RSP);
+};
+
+template <int NY, int A, int B, int NT, int RP_ = 8>
+__global__ void __launch_bounds__(NT)
+k_ybracket_t(const cplx* __restrict__ Zt, const cplx* __restrict__ R, cplx* __restrict__ P,
+             const cplx* __restrict__ tw_g, int Nx, int nzb, int vfast)
+{
+    constexpr int RP = RP_, A1 = A / 3, NKY0 = NY / 3, W2 = 2 * NKY0;
+    constexpr int BP = Tile<A, B>::BP, RS = YBracketT<NY, A, B, NT, RP_>::RSP;
+    extern __shared__ cplx smem[];
+    cplx* E = smem;
+    const int half = Nx / 2;
+    const int ntile = half / RP;
+    int bl, m0;
+    if (vfast) {
+        const int nvc = gridDim.x / (ntile * nzb);
+        m0 = ((blockIdx.x / nvc) % ntile) * RP;
+        bl = blockIdx.x / (nvc * ntile) + nzb * (blockIdx.x % nvc);
+    } else {
+        bl = blockIdx.x / ntile;
+        m0 = (blockIdx.x % ntile) * RP;
+    }
+    const int ql = bl % nzb;
+    const cplx* Zp = Zt + (size_t)bl * Nx * W2;
+
+    // Y1: pruned radix-A + twiddle; item = (row r of 16, n2), lanes over the rows
+    for (int item = threadIdx.x; item < 2 * RP * B; item += NT) {
+        const int r = item % (2 * RP), n2 = item / (2 * RP);
+        const int m = m0 + (r % RP) + (r / RP) * half;
+        cplx lo[A1], hi[A1];
+#pragma unroll
+        for (int a = 0; a < A1; ++a) {
+            lo[a] = __ldg(reinterpret_cast<const double2*>(Zp + (size_t)(n2 + B * a) * Nx + m));
+            hi[a] = __ldg(reinterpret_cast<const double2*>(Zp + (size_t)(n2 + B * a + NKY0) * Nx + m));
+        }
+        cplx out[A];
+        dft_pruned_in<A, +1>(lo, hi, out);
+        cplx* Er = E + r * RS + n2;
+#pragma unroll
+        for (int k1 = 0; k1 < A; ++k1) {
+            const cplx w = TWD_G(k1, n2);
+            Er[k1 * BP] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
+        }
+    }
+    __syncthreads();
+
+    // Y2: radix-B to real space for both rows of a pair, bracket, radix-B back + twiddle (in place)
+    for (int item = threadIdx.x; item < RP * A; item += NT) {
+        const int k1 = item % A, r = item / A;
+        cplx w[B];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const int row = r + h * RP;
+            const int m = m0 + r + h * half;
+            cplx v[B];
+            const cplx* Er = E + row * RS + k1 * BP;
+#pragma unroll
+            for (int n2 = 0; n2 < B; ++n2) v[n2] = Er[n2];
+            Dft<B, +1>::run(v);
+            const cplx* Rc = R + ((size_t)ql * Nx + m) * NY + k1;
+#pragma unroll
+            for (int k2 = 0; k2 < B; ++k2) {
+                const cplx c = Rc[A * k2];  // (dx chi, dy chi)
+                const double nl = fma(c.x, v[k2].y, -c.y * v[k2].x);
+                if (h == 0) w[k2].x = nl; else w[k2].y = nl;
+            }
+        }
+        Dft<B, -1>::run(w);
+        cplx* Er = E + r * RS + k1 * BP;
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) {
+            cplx tq = TWD_G(k1, k2);
+            Er[k2] = (k2 == 0) ? w[0] : cmul(w[k2], tq.x, -tq.y);
+        }
+    }
+    __syncthreads();
+
+    // Y3: pruned-output radix-A over n1 for fixed k2; j = k2 + B*k1
+    for (int item = threadIdx.x; item < RP * B; item += NT) {
+        const int k2 = item % B, r = item / B;
+        cplx in[A];
+        const cplx* Er = E + r * RS + k2;
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) in[n1] = Er[n1 * BP];
+        cplx lo[A1], hi[A1];
+        dft_pruned_out<A, -1>(in, lo, hi);
+        cplx* Pp = P + ((size_t)bl * half + m0 + r) * W2 + k2;
+#pragma unroll
+        for (int cq = 0; cq < A1; ++cq) {
+            Pp[B * cq] = lo[cq];
+            Pp[B * cq + NKY0] = hi[cq];
         }
     }
 }
