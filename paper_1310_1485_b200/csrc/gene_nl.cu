@@ -107,10 +107,13 @@ bool find_fused(int nx, int ny, FusedKernel* out)
 typedef void (*xinvp_fn)(const cplx*, cplx*, const cplx*, int, int, long long, double, double, int);
 struct XKernels {
     int nx, ck, nt;
+    int ck_inv = 0, nt_inv = 0;  // k_xinv's own tile width / threads when they differ from k_xfwd's (0: the same)
     size_t smem_inv, smem_fwd;
     xinv_fn inv;
     xfwd_fn fwd;
-    xinvp_fn invp_zt = nullptr;  // the same, storing Z transposed (for k_ybracket_t)
+    xinvp_fn invp_zt = nullptr;  // the same, storing Z transposed (for k_ybracket_t); may use fewer columns per tile
+    int ck_zt = 0;
+    size_t smem_invp_zt = 0;
     xinvp_fn invp = nullptr;  // pipelined persistent version (nl_pipe.cuh)
     size_t smem_invp = 0;
     int cap_invp = 0;         // its grid (resident CTAs); 0: use the first-generation kernel
@@ -124,6 +127,7 @@ struct YKernels {
     ybr_fn br_em;  // chi = phi_bar - v_par A_par_bar composed in the bracket
     ybrt_fn br_t = nullptr;  // g side read from the transposed Z (tiles of 8 row pairs, 128 threads)
     size_t smem_t = 0;
+    int rp_t = 8, nt_t = 128;
     ybrcv_fn br_cv;  // chi per plane: its y-synthesis fused into the bracket kernel (no R round trip)
     size_t smem_cv;
     int rp_cv;
@@ -140,7 +144,10 @@ XKernels make_x()
     k.inv = gnl::k_xinv<NX, A, B, CK, NT>;
     k.fwd = gnl::k_xfwd<NX, A, B, CK, NT>;
     k.invp = gnl::k_xinv_p<NX, A, B, CK, NT, false>;
-    k.invp_zt = gnl::k_xinv_p<NX, A, B, CK, NT, true>;
+    constexpr int CKZ = (NX >= 768) ? 2 : CK;  // transposed stores are 128 B runs for any CK: small tiles where smem is tight
+    k.invp_zt = gnl::k_xinv_p<NX, A, B, CKZ, NT, true>;
+    k.ck_zt = CKZ;
+    k.smem_invp_zt = gnl::XInvP<NX, A, B, CKZ, NT>::SMEM_BYTES;
     k.smem_invp = gnl::XInvP<NX, A, B, CK, NT>::SMEM_BYTES;
     return k;
 }
@@ -153,8 +160,10 @@ YKernels make_y()
     k.smem_real = k.smem_br;
     k.br = gnl::k_ybracket<NY, A, B, RP, NT, false>;
     k.br_em = gnl::k_ybracket<NY, A, B, RP, NT, true>;
-    k.br_t = gnl::k_ybracket_t<NY, A, B, 128, 8>;
-    k.smem_t = gnl::YBracketT<NY, A, B, 128, 8>::SMEM_BYTES;
+    constexpr int RPT = (NY >= 384) ? 4 : 8, NTT = (NY >= 384) ? 64 : 128;
+    k.br_t = gnl::k_ybracket_t<NY, A, B, NTT, RPT>;
+    k.smem_t = gnl::YBracketT<NY, A, B, NTT, RPT>::SMEM_BYTES;
+    k.rp_t = RPT; k.nt_t = NTT;
     constexpr int RPC = (RP >= 8) ? RP / 2 : RP;  // twice the exchange tiles per pair: fewer pairs per CTA
     k.br_cv = gnl::k_ybracket_cv<NY, A, B, RPC, NT>;
     k.smem_cv = sizeof(cplx) * (size_t)(4 * RPC * gnl::Tile<A, B>::FLAT);
@@ -172,7 +181,12 @@ bool find_x(int nx, XKernels* out)
     case 144: *out = make_x<144, 12, 12, 8, 128>(); return true;
     case 192: *out = make_x<192, 24, 8, 8, 128>(); return true;
     case 384: *out = make_x<384, 24, 16, 4, 128>(); return true;
-    case 768: *out = make_x<768, 24, 32, 4, 128>(); return true;
+    case 768: *out = make_x<768, 24, 32, 4, 128>();
+        // row-major Z in 128 B pieces: 8 columns per CTA, the two signs one after the other through the same 8 tiles
+        // of E (measured on B200, configs[3]: k_xinv 36.0 -> 32.7 ms)
+        out->inv = gnl::k_xinv<768, 24, 32, 8, 128, true>;
+        out->ck_inv = 8; out->nt_inv = 128;
+        return true;
     default: return false;
     }
 }
@@ -327,7 +341,7 @@ bool set_smem(K fn, size_t bytes, const char* name)
             GNL_LAUNCH(prof, K_XINV, (h->xk.invp<<<((ntiles) < h->xk.cap_invp ? (ntiles) : h->xk.cap_invp), h->xk.nt, h->xk.smem_invp, st>>>( \
                                          SRC, ZZ, h->twx, h->nky0, NZB, VSTR, h->kxmin, h->kymin, (ntiles))));                   \
         else                                                                                                                    \
-            GNL_LAUNCH(prof, K_XINV, (h->xk.inv<<<(ntiles), h->xk.nt, h->xk.smem_inv, st>>>(SRC, ZZ, h->twx, h->nky0, NZB, VSTR, h->kxmin, h->kymin))); \
+            GNL_LAUNCH(prof, K_XINV, (h->xk.inv<<<(h->xk.ck_inv ? (ntiles) * h->xk.ck / h->xk.ck_inv : (ntiles)), h->xk.nt_inv ? h->xk.nt_inv : h->xk.nt, h->xk.smem_inv, st>>>(SRC, ZZ, h->twx, h->nky0, NZB, VSTR, h->kxmin, h->kymin))); \
     } while (0)
 
 // Enqueue one chunk: planes (zi in [0,nzc), vi in [0,nv)), plane offset zi + vstride*vi from g/rhs;
@@ -379,9 +393,9 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
             launches += 2;
         }
         if (h->zt && !apar) {
-            const int ntot = nb * xt;
-            GNL_LAUNCH(prof, K_XINV, (xk.invp_zt<<<(ntot < h->cap_invp_zt ? ntot : h->cap_invp_zt), xk.nt, xk.smem_invp, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin, ntot)));
-            GNL_LAUNCH(prof, K_YBRACKET, (yk.br_t<<<nb * ((h->Nx / 2) / 8), 128, yk.smem_t, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, vfast)));
+            const int ntot = nb * (h->nky0 / xk.ck_zt);
+            GNL_LAUNCH(prof, K_XINV, (xk.invp_zt<<<(ntot < h->cap_invp_zt ? ntot : h->cap_invp_zt), xk.nt, xk.smem_invp_zt, st>>>(g + off, s.Z, h->twx, h->nky0, nzc, vstride, h->kxmin, h->kymin, ntot)));
+            GNL_LAUNCH(prof, K_YBRACKET, (yk.br_t<<<nb * ((h->Nx / 2) / yk.rp_t), yk.nt_t, yk.smem_t, st>>>(s.Z, s.R, s.P, h->twy, h->Nx, nzc, vfast)));
             GNL_LAUNCH(prof, K_XFWD, (xk.fwd<<<nb * xt, xk.nt, xk.smem_fwd, st>>>(s.P, rhs + off, h->twx, h->nky0, nzc, vstride, coef)));
             launches += 3;
             continue;
@@ -492,7 +506,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
         delete h;
         return nullptr;
     }
-    if (nky0 % h->xk.ck || (h->Nx / 2) % h->yk.rp || h->Nx % h->yk.rt) {
+    if (nky0 % h->xk.ck || (h->xk.ck_inv && nky0 % h->xk.ck_inv) || (h->Nx / 2) % h->yk.rp || h->Nx % h->yk.rt) {
         set_err("gene_nl_create: internal tiling does not divide the grid");
         delete h;
         return nullptr;
@@ -560,16 +574,16 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
             h->xk.cap_invp = occ * sms;
     }
-    if (ok && !h->chi_has_v && !h->em && !h->fused && (h->Nx / 2) % 8 == 0 && h->Ny <= 192 && h->yk.smem_t <= 227 * 1024 &&
-        h->xk.smem_invp <= 227 * 1024) {
+    if (ok && !h->chi_has_v && !h->em && !h->fused && (h->Nx / 2) % h->yk.rp_t == 0 && h->nky0 % h->xk.ck_zt == 0 &&
+        (h->Ny <= 192 || getenv("GENE_NL_ZT")) && h->yk.smem_t <= 227 * 1024 && h->xk.smem_invp_zt <= 227 * 1024) {
         // measured on B200: 384 x 192 (configs[2]) 7.79 -> 7.19 ms; at Ny = 384 the 105 KB of exchange tiles of
         // k_ybracket_t cost more than the stores save (configs[3]: 101 -> 119 ms), so that size keeps the row-major Z
         const char* e = getenv("GENE_NL_ZT");  // development knob
         int sms = 0, occ = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if ((e ? atoi(e) : 1) && set_smem(h->yk.br_t, h->yk.smem_t, "k_ybracket_t smem") &&
-            set_smem(h->xk.invp_zt, h->xk.smem_invp, "k_xinv_p<ZT> smem") &&
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp_zt, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0) {
+            set_smem(h->xk.invp_zt, h->xk.smem_invp_zt, "k_xinv_p<ZT> smem") &&
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp_zt, h->xk.nt, h->xk.smem_invp_zt) == cudaSuccess && occ > 0) {
             h->zt = true;
             h->cap_invp_zt = occ * sms;
         }

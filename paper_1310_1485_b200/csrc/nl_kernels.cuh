@@ -55,7 +55,9 @@ __device__ __forceinline__ void load_twiddles_ab(cplx* tw_s, const cplx* __restr
 // k_xinv: spectral plane F[ky][i]  ->  Z[bl][m][cc]   (x-synthesis of (i kx -+ ky) F, padded 3/2)
 // grid = planes_in_batch * (nky0 / CK); one CTA does CK stored columns = 2 CK FFTs of length NX.
 // ------------------------------------------------------------------------------------------------
-template <int NX, int A, int B, int CK, int NT>
+// SEQ: the +ky and the -ky transforms of the CK columns go through E one after the other, so E holds CK tiles
+// instead of 2*CK and twice as many columns fit (128 B instead of 64 B pieces in the row-major store of Z).
+template <int NX, int A, int B, int CK, int NT, bool SEQ = false>
 __global__ void __launch_bounds__(NT)
 k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restrict__ tw_g,
        int nky0, int nzb, long long vstride, double kxmin, double kymin)
@@ -76,11 +78,14 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
 
     load_twiddles_ab<A, B>(tw, tw_g);
     __syncthreads();
+    constexpr int NSG = SEQ ? 1 : 2;  // signs per pass through E
 
+#pragma unroll 1
+    for (int sg0 = 0; sg0 < 2; sg0 += NSG) {
     // stage 1: pruned radix-A over n1 for fixed n2 (n = n2 + B*n1), then twiddle W_NX^{n2 k1}
-    for (int item = threadIdx.x; item < 2 * CK * B; item += NT) {
+    for (int item = threadIdx.x; item < NSG * CK * B; item += NT) {
         const int n2 = item % B, c2 = item / B;
-        const int col = c2 % CK, sg = c2 / CK;
+        const int col = c2 % CK, sg = sg0 + c2 / CK;
         const int kyi = ky0 + col;
         if (sg == 1 && kyi == 0) continue;  // there is no -0 column
         const cplx* Fc = F + (size_t)kyi * NX0;
@@ -123,10 +128,10 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
     __syncthreads();
 
     // stage 2: radix-B over n2 for fixed k1; output m = k1 + A*k2
-    for (int item = threadIdx.x; item < 2 * CK * A; item += NT) {
+    for (int item = threadIdx.x; item < NSG * CK * A; item += NT) {
         const int col = item % CK, rest = item / CK;
-        const int k1 = rest % A, sg = rest / A;
-        const int c2 = sg * CK + col, kyi = ky0 + col;
+        const int k1 = rest % A, sg = sg0 + rest / A;
+        const int c2 = (rest / A) * CK + col, kyi = ky0 + col;
         const bool zero = (sg == 1 && kyi == 0);
         cplx v[B];
         const cplx* Ec = E + c2 * CS + k1 * BP;
@@ -140,6 +145,8 @@ k_xinv(const cplx* __restrict__ src, cplx* __restrict__ Z, const cplx* __restric
             const int m = k1 + A * k2;
             Zc[(size_t)m * W2] = sg ? cconj(v[k2]) : v[k2];
         }
+    }
+    if (SEQ && sg0 == 0) __syncthreads();  // stage 2 has read E before the -ky pass overwrites it
     }
 }
 
