@@ -40,6 +40,7 @@ SHAPES = [
     (128, 32, 3, 3, 1, 1, False), (128, 64, 1, 2, 1, 1, True),
     (256, 64, 2, 2, 1, 1, False), (32, 128, 1, 3, 1, 1, False),
     (512, 16, 1, 2, 1, 1, True), (16, 8, 1, 1, 1, 1, False),
+    (256, 64, 36, 2, 1, 1, False),   # chi rows of a chunk beyond 40 MB: the v-fastest tile walk of k_ybracket_t
 ]
 
 
