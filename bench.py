@@ -1,13 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- E x B nonlinearity planes/s on B200 (BASELINE.json metric), one JSON line on stdout.
 
-    python bench.py --gpus N --steps K --warmup W [--config 1] [--impl reference]
+    python bench.py --gpus N --steps K --warmup W [--config I] [--impl reference]
 
 A "step" is one pass of the whole hot path (gene_nl_compute: derivative + pad + to real space,
-bracket, back, delete modes, prefactor, add to rhs) over all planes of the workload.  At N = 1 the
-workload is BASELINE.json configs[1] (128x32 modes, 8192 planes, 512 MiB per array).  For N > 1
-(torchrun, one rank per GPU) every rank runs its own configs[1]-sized problem (planes are
-independent: weak scaling, no collective on the data path); the time is the max over ranks.
+bracket, back, delete modes, prefactor, add to rhs) over all planes of the workload.  The workload is
+BASELINE.json configs[3] (512x128 modes, 24 576 planes, 24 GiB per array): BASELINE.json's metric names
+no configuration, so the headline is the largest single-GPU one; with no --config the line also carries
+`per_config` = configs[1], [2], [4] measured device-resident in the same run.  For N > 1 (torchrun, one
+rank per GPU) every rank runs its own problem of that size (planes are independent: weak scaling, no
+collective on the data path); the time is the max over ranks.
 
 Keys beyond the base contract: `roofline` (dominant kernel, timed live with CUDA events on the
 launching stream through gene_nl_compute_profiled), `roofline_step` (whole step), `kernels`
@@ -59,7 +61,7 @@ class ClockSampler(threading.Thread):
     REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
                0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
 
-    def __init__(self, torch_index, period=0.02):
+    def __init__(self, torch_index, period=0.002):
         super().__init__(daemon=True)
         self.period, self.samples, self.reasons, self.max_mhz = period, [], set(), None
         self._halt = threading.Event()
@@ -255,32 +257,25 @@ def xglobal_main(args):
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     gbs = B * wl.planes / (ms_per_step * 1e-3) / 1e9     # the step IS one launch of k_xglobal
-    traffic = None
-    try:
-        import csv
-        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
-            if row["workload"] == "xglobal_64x16" and row["kernel"] == "k_xglobal":
-                traffic = float(row["dram_bytes_per_launch"]) * wl.planes / float(row["planes_per_launch"])
-    except Exception:
-        pass
+    cap, why = measured_traffic("xglobal_64x16")
+    traffic = cap["k_xglobal"][0] * wl.planes / cap["k_xglobal"][1] if "k_xglobal" in cap else None
     roofline = {"kernel": "k_xglobal", "bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
                 "frac": gbs / hbm_peak, "traffic": traffic,
+                "traffic_note": why or ("ncu --set full capture stamped with src_sha16 %s" % source_sha16()),
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
                 "bytes_per_plane": B, "flops_per_plane": F, "achieved_tflops": F * wl.planes / (ms_per_step * 1e-3) / 1e12,
                 "share_of_step": 1.0}
     # end to end: pinned host buffers, H2D of the five arrays and D2H of rhs inside the timed region (bounded slice)
     e2e = None
     if not args.no_e2e:
+        from paper_1310_1485_b200 import gene_nlx_compute_host
         n = min(wl.planes, 65536)
         host = [t[:n].cpu().pin_memory() for t in (vex, vey, dxg, dyg, rhs)]
-        devb = [torch.empty_like(t[:n]) for t in (vex, vey, dxg, dyg, rhs)]
+        hpref = pref.cpu()
         h2 = gene_nlx_create(wl.nx, wl.nky0, n)
 
-        def once():
-            for hb, db in zip(host, devb):
-                db.copy_(hb, non_blocking=True)
-            gene_nlx_compute(h2, devb[0], devb[1], devb[2], devb[3], pref, devb[4], wl.scale, stream)
-            host[4].copy_(devb[4], non_blocking=True)
+        def once():   # chunks of planes on three streams: H2D, kernel and D2H of different chunks overlap
+            gene_nlx_compute_host(h2, host[0], host[1], host[2], host[3], hpref, host[4], wl.scale)
         once()
         barrier()
         t0 = time.perf_counter()
@@ -290,7 +285,8 @@ def xglobal_main(args):
         dt = time.perf_counter() - t0
         e2e = {"value": n * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 5 * n * wl.plane_bytes,
                "d2h_bytes_per_step": n * wl.plane_bytes, "steps": args.e2e_steps,
-               "api": f"torch H2D of 5 arrays + gene_nlx_compute + D2H of rhs on {n} planes (pinned host buffers)"}
+               "api": f"gene_nlx_compute_host on {n} planes (pinned host buffers, chunked over three streams)",
+               "link_roofline_planes_per_s": None}
         gene_nlx_destroy(h2)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -382,15 +378,11 @@ def em_main(args):
                 "flops_per_plane": F, "bytes_per_plane": B}
     e2e = None
     if not args.no_e2e:   # pinned host buffers; H2D of g, rhs, phi, apar and D2H of rhs inside the timed region
+        from paper_1310_1485_b200 import gene_nl_compute_em_host
         host = [t.cpu().pin_memory() for t in (phi, apar, g, rhs)]
 
         def once():
-            phi.copy_(host[0], non_blocking=True)
-            apar.copy_(host[1], non_blocking=True)
-            g.copy_(host[2], non_blocking=True)
-            rhs.copy_(host[3], non_blocking=True)
-            gene_nl_compute_em(h, phi, apar, vpar, g, rhs, wl.scale, stream)
-            host[3].copy_(rhs, non_blocking=True)
+            gene_nl_compute_em_host(h, host[0], host[1], vpar, host[2], host[3], wl.scale)
         once()
         barrier()
         t0 = time.perf_counter()
@@ -401,7 +393,7 @@ def em_main(args):
         nb = sum(t.numel() * 16 for t in (phi, apar, g, rhs))
         e2e = {"value": wl.planes * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": nb,
                "d2h_bytes_per_step": rhs.numel() * 16, "steps": args.e2e_steps,
-               "api": "torch H2D of phi, apar, g, rhs + gene_nl_compute_em + D2H of rhs (pinned host buffers)"}
+               "api": "gene_nl_compute_em_host (pinned host buffers, one (w,s) slab per stage, three streams)"}
     launches = gene_nl_launches_per_compute(h)
     gene_nl_destroy(h)
     if rank == 0:
@@ -418,61 +410,56 @@ def em_main(args):
         dist.destroy_process_group()
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1)")
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--xglobal", action="store_true",
-                    help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
-    ap.add_argument("--strong", action="store_true",
-                    help="with --gpus N > 1: shard ONE problem's (w,s) slabs over the ranks instead of one problem per rank")
-    ap.add_argument("--em", action="store_true",
-                    help="chi composed on the device from phi_bar and A_par_bar (SURVEY 8(f) f1) on --config's grid")
-    ap.add_argument("--xglobal-planes", type=int, default=589824, help="planes per GPU (Table 4: 589824)")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 0)
-    if args.xglobal:
-        xglobal_main(args)
-        return
-    if args.em:
-        em_main(args)
-        return
+def source_sha16():
+    """sha256 over the CUDA sources: rows of profiles/dram_traffic.csv are stamped with it at capture time."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1310_1485_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
 
-    from paper_1310_1485_b200 import workloads as W
-    wl = W.CONFIGS[args.config]
-    if args.impl == "reference":
-        reference_arm(args, wl)
-        return
 
+def measured_traffic(workload_name):
+    """{kernel: (dram bytes per launch, planes per launch)} from the committed ncu capture, ONLY when the capture was
+    taken from the CUDA sources that are being timed now (src_sha16 column); else ({}, why)."""
+    import csv
+    rows, stale = {}, 0
+    try:
+        sha = source_sha16()
+        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
+            if row["workload"] != workload_name:
+                continue
+            if row.get("src_sha16", "") != sha:
+                stale += 1
+                continue
+            rows[row["kernel"]] = (float(row["dram_bytes_per_launch"]), float(row["planes_per_launch"]))
+    except Exception as e:  # noqa: BLE001
+        return {}, f"profiles/dram_traffic.csv unreadable: {e}"
+    if not rows:
+        return {}, ("capture predates the current CUDA sources" if stale else "no ncu capture for this workload")
+    return rows, None
+
+
+def run_config(wl, args, env, do_e2e, do_cpu, headline):
+    """Time one workload: device-resident steps (CUDA events on the launching stream, max over ranks), per-kernel
+    rooflines (event pair per launch), e2e through the host entry point, the oracle as cpu_baseline."""
     import torch
 
     from paper_1310_1485_b200 import GeneNL, gene_nl_probe_peaks
+    from paper_1310_1485_b200 import workloads as W
+    from paper_1310_1485_b200.binding import KERNEL_CLASSES
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=dev)
+    dev, dist, world, rank, local_rank = env["dev"], env["dist"], env["world"], env["rank"], env["local_rank"]
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    if args.strong and world > 1:
+    strong = args.strong and world > 1
+    if strong:
         # ONE problem of the workload's shape, its (w,s) slabs sharded over the ranks (SURVEY.md 8(e)/(f4)): g, rhs and
         # chi shard together, no exchange.  Each rank generates its own slabs (same recipe, rank-dependent seed).
         s0, s1 = W.shard_slabs(wl, rank, world)
@@ -486,14 +473,22 @@ def main():
     nl = GeneNL(my)
     stream = torch.cuda.current_stream()
     warm = max(args.warmup, 3)
-    for _ in range(warm):
+    w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    nl.compute(chi, g, rhs, stream=stream)
+    w0.record(stream)
+    for _ in range(warm - 1):
         nl.compute(chi, g, rhs, stream=stream)
+    w1.record(stream)
     barrier()
+    steps = args.steps
+    if not headline:   # side configs: at least half a second of timed work
+        est = max(w0.elapsed_time(w1) / (warm - 1), 1e-3)
+        steps = int(min(2000, max(args.steps, math.ceil(500.0 / est))))
     sampler = ClockSampler(local_rank)
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
-    for _ in range(args.steps):
+    for _ in range(steps):
         nl.compute(chi, g, rhs, stream=stream)
     e1.record(stream)
     barrier()
@@ -501,9 +496,7 @@ def main():
     ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device=dev)
     if dist is not None:
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_total = float(ms.item())
-    ms_per_step = ms_total / args.steps
-    strong = args.strong and world > 1
+    ms_per_step = float(ms.item()) / steps
     if strong:
         pt = torch.tensor([float(my.planes)], dtype=torch.float64, device=dev)
         dist.all_reduce(pt, op=dist.ReduceOp.SUM)
@@ -513,7 +506,6 @@ def main():
     value = planes_total / (ms_per_step * 1e-3)
 
     # per-kernel device time, live, with CUDA events on the launching stream
-    from paper_1310_1485_b200.binding import KERNEL_CLASSES
     prof_ms = {k: 0.0 for k in KERNEL_CLASSES}
     prof_n = dict.fromkeys(prof_ms, 0)
     nprof = 3
@@ -526,16 +518,13 @@ def main():
     if my.chi_has_v and not prof_n.get("k_yreal") and "k_yreal" in flops and "k_ybracket" in flops:
         flops["k_ybracket"] += flops.pop("k_yreal")  # chi's y-synthesis runs inside k_ybracket_cv (no k_yreal launches)
     fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
-    try:
-        probe_tf, probe_smem_gbs, _ = gene_nl_probe_peaks()
-    except Exception:
-        probe_tf, probe_smem_gbs = None, None
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    if "probe" not in env:
+        try:
+            env["probe"] = gene_nl_probe_peaks()
+        except Exception:  # noqa: BLE001
+            env["probe"] = (None, None, None)
+    probe_tf, probe_smem_gbs, _ = env["probe"]
+    hbm_peak = float(env["peaks"].get("hbm_gbs", 6650.0))
     kernels = {}
     for k in prof_ms:
         if prof_n[k]:
@@ -544,16 +533,16 @@ def main():
                           "avg_launch_us": 1e3 * avg_ms,
                           "tflops": flops[k] * nprof / (prof_ms[k] * 1e-3) / 1e12}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
-    traffic = None
-    try:  # measured DRAM bytes per launch of the dominant kernel, from the committed ncu capture
-        import csv
-        for row in csv.DictReader(open(os.path.join(ROOT, "profiles", "dram_traffic.csv"))):
-            if row["workload"] == wl.name and row["kernel"] == dom:
-                traffic = float(row["dram_bytes_per_launch"])
-    except Exception:
-        pass
+    # measured DRAM bytes (ncu capture of these very sources; null when the capture is older than the code)
+    cap, why = measured_traffic(wl.name)
+    traffic = cap[dom][0] if dom in cap else None
+    traffic_step = None
+    if cap and all(k in cap for k in kernels):
+        # whole step: every kernel's bytes per plane of its launch x the planes (chi planes for the chi-side kernels)
+        traffic_step = sum(cap[k][0] / cap[k][1] * (my.chi_planes if k == "k_yreal" else my.planes) for k in kernels)
     roofline = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
                 "unit": "TFLOP/s", "frac": kernels[dom]["tflops"] / fp64_model, "traffic": traffic,
+                "traffic_note": why or ("ncu --set full capture stamped with src_sha16 %s" % source_sha16()),
                 "peak_source": "model 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md sect. 7)",
                 "peak_measured_dfma": probe_tf, "smem_gbs_measured": probe_smem_gbs,
                 "share_of_step": kernels[dom]["ms_per_step"] / sum(v["ms_per_step"] for v in kernels.values())}
@@ -565,53 +554,150 @@ def main():
     roofline_step = {"bound": "alu" if t_alu >= t_hbm else "hbm", "achieved_tflops": step_tf,
                      "achieved_hbm_gbs": step_gbs, "peak_tflops": fp64_model, "peak_hbm_gbs": hbm_peak,
                      "roofline_planes_per_s": roof_planes, "frac": (value / world) / roof_planes,
-                     "flops_per_plane": F, "bytes_per_plane": B}
-
-    # end to end through the host entry point: pinned host buffers, copies inside the timed region
-    e2e = None
-    if not args.no_e2e:
-        hchi, hg, hrhs = (t.cpu().pin_memory() for t in (chi, g, rhs))
-        nl.compute_host(hchi, hg, hrhs)   # warm-up (allocates staging)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            nl.compute_host(hchi, hg, hrhs)
-        torch.cuda.synchronize()
-        dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
-        gb = my.plane_bytes * my.planes
-        e2e = {"value": planes_total * args.e2e_steps / float(dt.item()), "unit": UNIT,
-               "h2d_bytes_per_step": 2 * gb + my.plane_bytes * my.chi_planes, "d2h_bytes_per_step": gb,
-               "steps": args.e2e_steps, "api": "gene_nl_compute_host (pinned host buffers)"}
-        del hchi, hg, hrhs
-
-    launches = nl.launches_per_compute * args.steps
+                     "frac_of_measured_dfma": (step_tf / probe_tf) if probe_tf else None,
+                     "flops_per_plane": F, "bytes_per_plane": B, "algorithmic_bytes_per_step": B * my.planes,
+                     "traffic_per_step": traffic_step}
+    launches = nl.launches_per_compute * steps
     nl.close()
 
+    # end to end through the host entry point: pinned host buffers, copies inside the timed region.  Arrays beyond
+    # 8 GiB (configs[3]: 49 GiB of g + rhs) are represented by their first (w,s) slabs -- the host entry point streams
+    # slab by slab, so the rate per plane is that of the whole array.
+    e2e = None
+    if do_e2e:
+        nslab = my.nw * my.nspec
+        slab_bytes = 2 * my.plane_bytes * my.nz * my.nv
+        ns = int(max(1, min(nslab, (8 << 30) // slab_bytes)))
+        sub, hchi, hg, hrhs = my, chi, g, rhs
+        if ns < nslab:
+            sub = W.Workload(f"{my.name}_first{ns}slabs", my.nx0, my.nky0, my.nz, my.nv, ns, 1, my.kxmin, my.kymin,
+                             my.chi_has_v, my.seed, my.rhs_random, my.scale)
+            hg = g.reshape((nslab,) + my.g_shape[2:])[:ns]
+            hrhs = rhs.reshape((nslab,) + my.g_shape[2:])[:ns]
+            hchi = chi.reshape((nslab,) + my.chi_shape[2:])[:ns]
+        hchi, hg, hrhs = (t.cpu().pin_memory() for t in (hchi, hg, hrhs))
+        del chi, g, rhs
+        torch.cuda.empty_cache()
+        with GeneNL(sub) as nlh:
+            nlh.compute_host(hchi, hg, hrhs)   # warm-up (allocates staging)
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(args.e2e_steps):
+                nlh.compute_host(hchi, hg, hrhs)
+            torch.cuda.synchronize()
+            dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(dt, op=dist.ReduceOp.MAX)
+        gb = sub.plane_bytes * sub.planes
+        e2e = {"value": sub.planes * world * args.e2e_steps / float(dt.item()), "unit": UNIT,
+               "h2d_bytes_per_step": 2 * gb + sub.plane_bytes * sub.chi_planes, "d2h_bytes_per_step": gb,
+               "steps": args.e2e_steps,
+               "api": "gene_nl_compute_host (pinned host buffers)" +
+                      ("" if ns == nslab else f" on the first {ns} of {nslab} (w,s) slabs = {sub.planes} planes per step")}
+        del hchi, hg, hrhs
+    else:
+        del chi, g, rhs
+    torch.cuda.empty_cache()
+
     cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if do_cpu and rank == 0 and world == 1:
         import oracle
         threads = oracle.num_threads()
         v, n, dt = time_oracle(wl, args.cpu_seconds / max(threads, 1), threads)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                         "sample": f"{n} planes of {wl.name} (first planes, up to four (w,s) slabs), {dt:.1f} s wall"}
+    return {
+        "value": value, "steps": steps, "warmup": warm, "ms_per_step": ms_per_step, "scaling": "strong" if strong else "weak",
+        "config": {"workload": wl.name, "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": my.planes,
+                   "padded_grid": [wl.Nx, wl.Ny], "chi_has_v": wl.chi_has_v,
+                   "cache": "inputs larger than L2 (g+rhs+chi = %.0f MiB per GPU)" %
+                            ((2 * my.planes + my.chi_planes) * my.plane_bytes / 2 ** 20),
+                   "parallelism": (f"one problem, (w,s) slabs sharded over {world} GPUs" if strong
+                                   else f"planes x{world} (independent problems per GPU)")},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "roofline_step": roofline_step,
+        "kernels": kernels, "cpu_baseline": cpu_baseline,
+    }
 
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=None,
+                    help="index into BASELINE.json configs.  Default: configs[3] (the largest single-GPU configuration: "
+                         "the headline) with a per_config block for configs[1], [2], [4] measured in the same run")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="CPU work of the cpu_baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="headline configuration only")
+    ap.add_argument("--xglobal", action="store_true",
+                    help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
+    ap.add_argument("--strong", action="store_true",
+                    help="with --gpus N > 1: shard ONE problem's (w,s) slabs over the ranks instead of one problem per rank")
+    ap.add_argument("--em", action="store_true",
+                    help="chi composed on the device from phi_bar and A_par_bar (SURVEY 8(f) f1) on --config's grid")
+    ap.add_argument("--xglobal-planes", type=int, default=589824, help="planes per GPU (Table 4: 589824)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    headline_idx = 3 if args.config is None else args.config
+    if args.xglobal:
+        xglobal_main(args)
+        return
+    if args.em:
+        args.config = 4 if args.config is None else args.config
+        em_main(args)
+        return
+
+    from paper_1310_1485_b200 import workloads as W
+    wl = W.CONFIGS[headline_idx]
+    if args.impl == "reference":
+        reference_arm(args, wl)
+        return
+
+    import torch
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:  # noqa: BLE001
+        pass
+    env = {"dev": dev, "dist": dist, "world": world, "rank": rank, "local_rank": local_rank, "peaks": peaks}
+
+    res = run_config(wl, args, env, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, headline=True)
+    per_config = None
+    if args.config is None and world == 1 and not args.no_per_config:
+        # the other target configurations, device-resident, in the same run (same box, same clocks record)
+        per_config = {}
+        for idx in (1, 2, 4):
+            r = run_config(W.CONFIGS[idx], args, env, do_e2e=False, do_cpu=False, headline=False)
+            per_config[W.CONFIGS[idx].name] = {k: r[k] for k in ("value", "ms_per_step", "steps", "roofline",
+                                                                  "roofline_step", "kernels", "clocks", "gpu_launches")}
+            per_config[W.CONFIGS[idx].name]["unit"] = UNIT
     if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": warm, "ms_per_step": ms_per_step, "higher_is_better": True,
-            "scaling": "strong" if strong else "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": wl.name, "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": my.planes,
-                       "padded_grid": [wl.Nx, wl.Ny], "chi_has_v": wl.chi_has_v,
-                       "cache": "inputs larger than L2 (g+rhs+chi = %.0f MiB per GPU)" %
-                                ((2 * my.planes + my.chi_planes) * my.plane_bytes / 2 ** 20),
-                       "parallelism": (f"one problem, (w,s) slabs sharded over {world} GPUs" if strong else f"planes x{world} (independent problems per GPU)")},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
-            "roofline": roofline, "roofline_step": roofline_step, "kernels": kernels,
-            "cpu_baseline": cpu_baseline,
+            "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": res["steps"],
+            "warmup": res["warmup"], "ms_per_step": res["ms_per_step"], "higher_is_better": True,
+            "scaling": res["scaling"], "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": res["config"], "clocks": res["clocks"], "e2e": res["e2e"], "gpu_launches": res["gpu_launches"],
+            "roofline": res["roofline"], "roofline_step": res["roofline_step"], "kernels": res["kernels"],
+            "cpu_baseline": res["cpu_baseline"],
         }
+        if per_config is not None:
+            line["per_config"] = per_config
         print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

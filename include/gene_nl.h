@@ -76,30 +76,22 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, 
  * keeping the amount of transfer constant").  For a plan created with chi_has_v = GENE_NL_CHI_EM:
  *     rhs[.,.,p] += scale * N(chi_p, g_p),   chi_p = phi_bar[z,w,s] - vpar[v + nv*s] * apar_bar[z,w,s],  p = (z,v,w,s).
  * phi, apar: DEVICE arrays, complex128 [nx0, nky0, nz, nw, nspec] (the layout of chi without v); vpar: HOST array of
- * nv*nspec doubles (copied on `stream`; it may be reused by the caller when the call returns).  By linearity the two
- * fields are transformed to real space once per (z,w,s) and combined inside the bracket kernel, so the per-plane chi
- * array (as large as g) is never formed, read or transformed.  Other arguments, errors and asynchrony as
- * gene_nl_compute.  Always the batched kernels.  gene_nl_compute / gene_nl_compute_host reject such a plan.
+ * nv*nspec doubles, pageable or pinned: it is copied into a plan-owned pinned staging buffer before the call returns
+ * (the caller may reuse it at once) and from there to the device on `stream`.  Because that staging buffer is reused,
+ * a call first waits on the host for the previous call's copy, and the call is NOT capturable in a CUDA graph
+ * (gene_nl_compute is).  By linearity the two fields are transformed to real space once per (z,w,s) and combined
+ * inside the bracket kernel, so the per-plane chi array (as large as g) is never formed, read or transformed.  Other
+ * arguments, errors and asynchrony as gene_nl_compute.  Always the batched kernels.  gene_nl_compute /
+ * gene_nl_compute_host reject such a plan.
  */
 #define GENE_NL_CHI_EM 2
 int gene_nl_compute_em(gene_nl_plan* h, const void* phi, const void* apar, const double* vpar_host, const void* g,
                        void* rhs, double scale, void* stream);
 
-/*
- * gene_nl_compute_profiled -- gene_nl_compute with a CUDA-event pair recorded on `stream` around every
- * kernel launch, then a stream synchronise.  ms[c] receives the summed device time [ms] and
- * launches[c] the launch count of kernel class c (arrays of GENE_NL_KERNEL_CLASSES entries):
- *   0 k_xinv       x-synthesis: derivative + pad + x half of the transform to real space
- *   1 k_yreal      chi real-space fields (dx chi, dy chi)
- *   2 k_ybracket   y-synthesis + bracket + y-analysis           (batched path, large planes)
- *   3 k_xfwd       x-analysis + delete modes + prefactor + add  (batched path, large planes)
- *   4 k_plane_fused  the whole g-side of a plane in one persistent kernel, x<->y hand-over in shared
- *                  memory (planes with Nx <= 192 and Ny <= 96)
- * Used by bench.py for per-kernel rooflines.
- */
-#define GENE_NL_KERNEL_CLASSES 5
-int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, void* rhs, double scale,
-                             void* stream, double* ms, int* launches);
+/* gene_nl_compute_em_host -- gene_nl_compute_em on HOST buffers (phi, apar, g, rhs; layouts as above), streamed through
+ * the device one (w,s) slab at a time exactly as gene_nl_compute_host does.  SYNCHRONOUS. */
+int gene_nl_compute_em_host(gene_nl_plan* h, const void* phi_host, const void* apar_host, const double* vpar_host,
+                            const void* g_host, void* rhs_host, double scale);
 
 /*
  * gene_nl_compute_host -- same operation on HOST buffers (same layouts).  The arrays are streamed
@@ -121,6 +113,16 @@ const char* gene_nl_last_error(void);
 /* Bytes of device scratch + tables owned by the plan. */
 size_t gene_nl_workspace_bytes(const gene_nl_plan* h);
 
+/*
+ * gene_nl_set_scratch_bytes -- change the plan's scratch budget (SURVEY.md 8(b) "optional workspace" extension).
+ * The planes of one compute are walked in batches whose scratch (the half-transformed arrays Z and P and the
+ * real-space chi fields) fits `bytes` per scratch set; the default is 768 MiB.  A smaller budget means more and
+ * smaller launches (and ragged last batches), never a different result.  Synchronises the device, frees and
+ * re-allocates the scratch (and drops the staging buffers of the host entry points).  bytes >= 1 MiB.
+ * Returns GENE_NL_OK, or GENE_NL_ENOMEM with the previous budget restored.
+ */
+int gene_nl_set_scratch_bytes(gene_nl_plan* h, size_t bytes);
+
 /* Number of kernel launches one gene_nl_compute enqueues (for launch accounting in benchmarks). */
 int gene_nl_launches_per_compute(const gene_nl_plan* h);
 
@@ -133,15 +135,6 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
  *   Returns NaN for an unknown `what` or NULL plan.
  */
 double gene_nl_query(const gene_nl_plan* h, int what);
-
-/*
- * gene_nl_probe_peaks -- micro-benchmarks of the two units that bound this path, on the current
- * device (used by bench.py for the roofline denominators; SURVEY.md 8(d) asks for a measured FP64
- * peak).  out[0] = FP64 DFMA throughput [TFLOP/s] from independent register-resident FMA chains on
- * all SMs; out[1] = shared-memory bandwidth [GB/s] from conflict-free 128-bit loads+stores on all
- * SMs; out[2] = SM clock [MHz] reported by the driver at the end of the probe.  Returns 0 on success.
- */
-int gene_nl_probe_peaks(double* out3);
 
 /* =====================================================================================================
  * x-GLOBAL VARIANT -- the operator the paper itself ran and timed (PAPER.md:39,
@@ -161,6 +154,10 @@ int gene_nl_probe_peaks(double* out3);
  * All pointers are DEVICE pointers, caller-owned, 16-byte aligned (pref: 8); rhs must not overlap an input.
  * Supported: nky0 in {8, 16, 32} (Ny = 24, 48, 96); any nx >= 1 (tiles of 16 x points, ragged tail allowed).
  * Asynchronous on `stream`; one kernel launch per compute.  Errors as for gene_nl_* (gene_nl_last_error).
+ * gene_nlx_compute_host takes HOST pointers (same layouts; pref a host array of nx doubles) and streams the planes
+ * through the device in chunks on three CUDA streams ("we split each input array into (usually four)
+ * contiguous chunks of xy-planes, which are transferred and computed in two asynchronous CUDA streams"); 5 planes go
+ * in and 1 comes out per plane computed.  SYNCHRONOUS; pinned host memory gives full overlap.
  * ===================================================================================================== */
 typedef struct gene_nlx_plan gene_nlx_plan;
 
@@ -169,6 +166,9 @@ gene_nlx_plan* gene_nlx_create(int nx, int nky0, long long planes);
 
 int gene_nlx_compute(gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
                      const double* pref, void* rhs, double scale, void* stream);
+
+int gene_nlx_compute_host(gene_nlx_plan* h, const void* vex_host, const void* vey_host, const void* dxg_host,
+                          const void* dyg_host, const double* pref_host, void* rhs_host, double scale);
 
 /* NULL is a no-op.  Synchronises the device. */
 void gene_nlx_destroy(gene_nlx_plan* h);

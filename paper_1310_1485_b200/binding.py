@@ -15,14 +15,15 @@ from . import build as _build
 
 GENE_NL_OK, GENE_NL_EINVAL, GENE_NL_EUNSUPPORTED, GENE_NL_ECUDA, GENE_NL_ENOMEM = 0, 1, 2, 3, 4
 
-# every symbol include/gene_nl.h declares
+# every symbol include/gene_nl.h declares (the product boundary) ...
 EXPORTED_SYMBOLS = (
-    "gene_nl_create", "gene_nl_compute", "gene_nl_compute_em", "gene_nl_compute_profiled", "gene_nl_compute_host",
-    "gene_nl_destroy",
-    "gene_nl_last_error",
-    "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query", "gene_nl_probe_peaks",
-    "gene_nlx_create", "gene_nlx_compute", "gene_nlx_destroy", "gene_nlx_query",
+    "gene_nl_create", "gene_nl_compute", "gene_nl_compute_em", "gene_nl_compute_host", "gene_nl_compute_em_host",
+    "gene_nl_destroy", "gene_nl_last_error", "gene_nl_set_scratch_bytes",
+    "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query",
+    "gene_nlx_create", "gene_nlx_compute", "gene_nlx_compute_host", "gene_nlx_destroy", "gene_nlx_query",
 )
+# ... and include/gene_nl_bench.h (benchmark-only helpers, not on the hot path)
+BENCH_SYMBOLS = ("gene_nl_compute_profiled", "gene_nl_probe_peaks")
 
 _lock = threading.Lock()
 _lib = None
@@ -57,6 +58,10 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_compute_profiled.restype = i
         lib.gene_nl_compute_host.argtypes = [vp, vp, vp, vp, dbl]
         lib.gene_nl_compute_host.restype = i
+        lib.gene_nl_compute_em_host.argtypes = [vp, vp, vp, ctypes.POINTER(dbl), vp, vp, dbl]
+        lib.gene_nl_compute_em_host.restype = i
+        lib.gene_nl_set_scratch_bytes.argtypes = [vp, ctypes.c_size_t]
+        lib.gene_nl_set_scratch_bytes.restype = i
         lib.gene_nl_destroy.argtypes = [vp]
         lib.gene_nl_destroy.restype = None
         lib.gene_nl_last_error.argtypes = []
@@ -74,6 +79,8 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nlx_create.restype = vp
         lib.gene_nlx_compute.argtypes = [vp, vp, vp, vp, vp, vp, vp, dbl, vp]
         lib.gene_nlx_compute.restype = i
+        lib.gene_nlx_compute_host.argtypes = [vp, vp, vp, vp, vp, vp, vp, dbl]
+        lib.gene_nlx_compute_host.restype = i
         lib.gene_nlx_destroy.argtypes = [vp]
         lib.gene_nlx_destroy.restype = None
         lib.gene_nlx_query.argtypes = [vp, i]
@@ -130,6 +137,22 @@ def gene_nl_compute_em(h, phi, apar, vpar, g, rhs, scale, stream=None) -> None:
                                            int(stream) or None)
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_compute_em failed ({rc}): {gene_nl_last_error()}")
+
+
+def gene_nl_compute_em_host(h, phi, apar, vpar, g, rhs, scale) -> None:
+    """gene_nl_compute_em on HOST arrays (torch CPU tensors, ideally pinned, or raw addresses); synchronous."""
+    vals = [float(x) for x in vpar]
+    arr = (ctypes.c_double * len(vals))(*vals)
+    rc = load_library().gene_nl_compute_em_host(h, _ptr(phi), _ptr(apar), arr, _ptr(g), _ptr(rhs), float(scale))
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_compute_em_host failed ({rc}): {gene_nl_last_error()}")
+
+
+def gene_nl_set_scratch_bytes(h, nbytes: int) -> None:
+    """Change the plan's scratch budget (bytes per scratch set); more, smaller batches -- never a different result."""
+    rc = load_library().gene_nl_set_scratch_bytes(h, int(nbytes))
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_set_scratch_bytes failed ({rc}): {gene_nl_last_error()}")
 
 
 KERNEL_CLASSES = ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd", "k_plane_fused")
@@ -205,6 +228,14 @@ def gene_nlx_compute(h, vex, vey, dxg, dyg, pref, rhs, scale, stream=None) -> No
         raise GeneNLError(f"gene_nlx_compute failed ({rc}): {gene_nl_last_error()}")
 
 
+def gene_nlx_compute_host(h, vex, vey, dxg, dyg, pref, rhs, scale) -> None:
+    """Same on HOST arrays (torch CPU tensors, ideally pinned, or raw addresses), chunked over CUDA streams; synchronous."""
+    rc = load_library().gene_nlx_compute_host(h, _ptr(vex), _ptr(vey), _ptr(dxg), _ptr(dyg), _ptr(pref), _ptr(rhs),
+                                              float(scale))
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nlx_compute_host failed ({rc}): {gene_nl_last_error()}")
+
+
 def gene_nlx_destroy(h) -> None:
     if h:
         load_library().gene_nlx_destroy(h)
@@ -217,9 +248,11 @@ def gene_nlx_query(h, what: int) -> float:
 class GeneNL:
     """Context-manager convenience around create/compute/destroy for a workloads.Workload."""
 
-    def __init__(self, wl):
+    def __init__(self, wl, scratch_bytes=None):
         self.wl = wl
         self.h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, wl.chi_has_v)
+        if scratch_bytes is not None:
+            gene_nl_set_scratch_bytes(self.h, scratch_bytes)
 
     def compute(self, chi, g, rhs, scale=None, stream=None):
         gene_nl_compute(self.h, chi, g, rhs, self.wl.scale if scale is None else scale, stream)

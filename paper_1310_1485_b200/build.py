@@ -25,7 +25,7 @@ def is_stale() -> bool:
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
-    deps.append(os.path.join(HERE, "..", "include", "gene_nl.h"))
+    deps += [os.path.join(HERE, "..", "include", f) for f in ("gene_nl.h", "gene_nl_bench.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 
@@ -34,8 +34,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not is_stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    extra = os.environ.get("GENE_NL_NVCC_EXTRA", "").split()  # development knob (e.g. -DGNL_EXP_...)
-    cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
         ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:

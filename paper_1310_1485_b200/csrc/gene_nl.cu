@@ -1,10 +1,11 @@
 // gene_nl.cu -- C ABI (include/gene_nl.h): plan, batching, launch sequence, host streaming driver.
 //
 // One gene_nl_compute walks the phase space in CHUNKS = (w,s) slab x z-range x all v, and inside a
-// chunk in BATCHES of v so that the per-batch scratch (Z, P, Rchi; see nl_kernels.cuh) stays in L2.
-// With chi_has_v = 0 the real-space chi fields of a chunk are formed once and reused by every v
-// (SURVEY.md 7 "chi reuse").  The host entry point streams chunks over several CUDA streams
-// (PAPER.md:69).
+// chunk in BATCHES of v whose scratch (Z, P, Rchi; see nl_kernels.cuh) fits the plan's scratch budget
+// (default 768 MiB per set -- far beyond the 126 MB L2 on purpose: measured on B200, long launches beat
+// L2-sized batches; gene_nl_set_scratch_bytes changes it).  With chi_has_v = 0 the real-space chi
+// fields of a chunk are formed once and reused by every v (SURVEY.md 7 "chi reuse").  The host entry
+// points stream (w,s) slabs over several CUDA streams.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -15,7 +16,7 @@
 #include <string>
 #include <vector>
 
-#include "../../include/gene_nl.h"
+#include "../../include/gene_nl_bench.h"
 #include "nl_fused.cuh"
 #include "nl_fused2.cuh"
 #include "nl_kernels.cuh"
@@ -236,7 +237,7 @@ struct Profiler {
 
 struct HostStage {  // per-stream staging of one chunk for gene_nl_compute_host
     cudaStream_t stream = nullptr;
-    cplx *g = nullptr, *rhs = nullptr, *chi = nullptr;
+    cplx *g = nullptr, *rhs = nullptr, *chi = nullptr, *apar = nullptr;
     Scratch scr;
 };
 
@@ -267,27 +268,22 @@ struct gene_nl_plan {
     size_t table_bytes;
     std::vector<HostStage> stages;  // lazily created by gene_nl_compute_host
     int device;
+    size_t budget = (size_t)768 << 20;  // scratch budget per set (gene_nl_set_scratch_bytes)
+    bool budget_set = false;            // explicit budget: it also bounds the fused path's chi cache
+    double* vp_pinned = nullptr;        // em: host staging of v_par (pinned), guarded by vp_event
+    cudaEvent_t vp_event = nullptr;
 };
 
 namespace {
 
-size_t scratch_budget_bytes()
+bool alloc_scratch(size_t zbytes, size_t pbytes, size_t rbytes, Scratch* s)
 {
-    // tuning knob (development): scratch budget per set in MiB.  Measured on B200: launches of several hundred
-    // planes amortise their tails better than L2-sized batches gain from staying in the 126 MB L2
-    const char* e = getenv("GENE_NL_SCRATCH_MB");
-    long mb = e ? atol(e) : 768;
-    if (mb < 1) mb = 1;
-    return (size_t)mb << 20;
-}
-
-bool alloc_scratch(gene_nl_plan* h, Scratch* s)
-{
-    if (!cuda_ok(cudaMalloc(&s->Z, h->zbytes), "cudaMalloc(Z)")) return false;
-    if (!cuda_ok(cudaMalloc(&s->P, h->pbytes), "cudaMalloc(P)")) return false;
-    if (!cuda_ok(cudaMalloc(&s->R, h->rbytes), "cudaMalloc(Rchi)")) return false;
+    if (!cuda_ok(cudaMalloc(&s->Z, zbytes), "cudaMalloc(Z)")) return false;
+    if (!cuda_ok(cudaMalloc(&s->P, pbytes), "cudaMalloc(P)")) return false;
+    if (!cuda_ok(cudaMalloc(&s->R, rbytes), "cudaMalloc(Rchi)")) return false;
     return true;
 }
+bool alloc_scratch(gene_nl_plan* h, Scratch* s) { return alloc_scratch(h->zbytes, h->pbytes, h->rbytes, s); }
 void free_scratch(Scratch* s)
 {
     cudaFree(s->Z); cudaFree(s->P); cudaFree(s->R);
@@ -322,6 +318,50 @@ bool upload_const_twiddles()
         }
     }
     return cuda_ok(cudaMemcpyToSymbol(gnl::c_tw, t.data(), sizeof(cplx) * t.size()), "cudaMemcpyToSymbol(twiddles)");
+}
+
+// Batching for the plan's scratch budget.  Batched path: chunk = nzb z-planes x all v; batch = nzb x nvb planes whose
+// scratch set fits the budget.  Fused path: nss (w,s) slabs per launch (their real-space chi is kept), nbz chi planes
+// per k_xinv / k_yreal batch.  Sets nzb, nvb, nss, nbz and the byte sizes of one scratch set.
+void configure_batching(gene_nl_plan* h)
+{
+    const int nz = h->nz, nv = h->nv;
+    const size_t W2 = 2 * (size_t)h->nky0;
+    const size_t zpp = sizeof(cplx) * h->Nx * W2, ppp = zpp / 2, rpp = sizeof(cplx) * (size_t)h->Nx * h->Ny;
+    const size_t budget = h->budget;
+    if (h->fused) {
+        const size_t cps = (size_t)nz * (h->chi_has_v ? nv : 1);          // chi planes per slab
+        const size_t rcap = h->budget_set ? budget : (size_t)2 << 30;     // real-space chi kept per launch
+        size_t nss = rcap / (cps * rpp);
+        if (nss < 1) nss = 1;
+        if (nss > (size_t)h->nw * h->nspec) nss = (size_t)h->nw * h->nspec;
+        h->nss = (int)nss;
+        const size_t zcap = (h->budget_set && budget < ((size_t)64 << 20)) ? budget : (size_t)64 << 20;
+        size_t nbz = zcap / zpp;
+        if (nbz < 1) nbz = 1;
+        if (nbz > cps * nss) nbz = cps * nss;
+        h->nbz = (long long)nbz;
+        h->nzb = nz; h->nvb = nv;
+        h->zbytes = zpp * nbz;
+        h->pbytes = 256;
+        h->rbytes = rpp * cps * nss;
+        return;
+    }
+    int nzb = nz;
+    if (!h->chi_has_v) {
+        while (nzb > 1 && (size_t)nzb * rpp * (h->em ? 2 : 1) > budget / 4) nzb = (nzb + 1) / 2;
+    }
+    const size_t per_plane = zpp + ppp + (h->chi_has_v ? rpp : 0);
+    while (nzb > 1 && (size_t)nzb * per_plane > budget / 2) nzb = (nzb + 1) / 2;
+    const size_t fixed = h->chi_has_v ? 0 : (size_t)nzb * rpp * (h->em ? 2 : 1);
+    long long nvb = (long long)((budget > fixed ? budget - fixed : 0) / ((size_t)nzb * per_plane));
+    if (nvb < 1) nvb = 1;
+    if (nvb > nv) nvb = nv;
+    h->nzb = nzb; h->nvb = (int)nvb;
+    const size_t nb = (size_t)nzb * nvb;
+    h->zbytes = zpp * nb;
+    h->pbytes = ppp * nb;
+    h->rbytes = rpp * (h->chi_has_v ? nb : (size_t)nzb * (h->em ? 2 : 1));
 }
 
 template <class K>
@@ -414,7 +454,7 @@ int enqueue_chunk(gene_nl_plan* h, const Scratch& s, const cplx* chi, long long 
 
 // Enqueue `nslab` contiguous (w,s) slabs (standard strides: v stride nz planes).  Returns launches or -1.
 int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx* g, cplx* rhs, int nslab,
-                  double scale, cudaStream_t st, Profiler* prof = nullptr, const cplx* apar = nullptr)
+                  double scale, cudaStream_t st, Profiler* prof = nullptr, const cplx* apar = nullptr, int slab0 = 0)
 {
     int launches = 0;
     if (h->fused) {
@@ -454,7 +494,7 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const size_t coff = h->chi_has_v ? goff : ((size_t)z0 + (size_t)h->nz * sl) * h->M;
             // em: slab sl = w + nw * species; its v_par coefficients are vp_dev[nv * species ..]
             int n = enqueue_chunk(h, sc, chi + coff, h->nz, g + goff, rhs + goff, h->nz, nzc, scale, str, prof,
-                                  apar ? apar + coff : nullptr, apar ? h->vp_dev + (size_t)h->nv * (sl / h->nw) : nullptr);
+                                  apar ? apar + coff : nullptr, apar ? h->vp_dev + (size_t)h->nv * ((slab0 + sl) / h->nw) : nullptr);
             if (n < 0) return -1;
             launches += n;
         }
@@ -511,50 +551,15 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
         delete h;
         return nullptr;
     }
-    // batching: chunk = nzb z-planes x all v; batch = nzb x nvb planes with scratch within the budget
-    const size_t W2 = 2 * (size_t)nky0;
-    const size_t zpp = sizeof(cplx) * h->Nx * W2, ppp = zpp / 2, rpp = sizeof(cplx) * (size_t)h->Nx * h->Ny;
-    const size_t budget = scratch_budget_bytes();
-    int nzb = nz;
-    if (!h->chi_has_v) {
-        while (nzb > 1 && (size_t)nzb * rpp * (h->em ? 2 : 1) > budget / 4) nzb = (nzb + 1) / 2;
-    }
-    const size_t per_plane = zpp + ppp + (h->chi_has_v ? rpp : 0);
-    while (nzb > 1 && (size_t)nzb * per_plane > budget / 2) nzb = (nzb + 1) / 2;
-    const size_t fixed = h->chi_has_v ? 0 : (size_t)nzb * rpp * (h->em ? 2 : 1);
-    long long nvb = (long long)((budget > fixed ? budget - fixed : 0) / ((size_t)nzb * per_plane));
-    if (nvb < 1) nvb = 1;
-    if (nvb > nv) nvb = nv;
-    h->nzb = nzb; h->nvb = (int)nvb;
-    const size_t nb = (size_t)nzb * nvb;
-    h->zbytes = zpp * nb;
-    h->pbytes = ppp * nb;
-    h->rbytes = rpp * (h->chi_has_v ? nb : (size_t)nzb * (h->em ? 2 : 1));
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
-    {
-        const char* e = getenv("GENE_NL_NO_FUSED");  // development knob: force the batched kernels
-        const char* e1 = getenv("GENE_NL_FUSED_V1");  // development knob: first-generation fused kernel
-        const bool want = !(e && atoi(e)) && !h->em;  // the composition lives in k_ybracket (batched path)
-        h->fused = want && ((!(e1 && atoi(e1)) && find_fused2(h->Nx, h->Ny, &h->fk)) || find_fused(h->Nx, h->Ny, &h->fk));
-    }
+    // the composition chi = phi_bar - v_par A_par_bar lives in k_ybracket (batched path)
+    h->fused = !h->em && (find_fused2(h->Nx, h->Ny, &h->fk) || find_fused(h->Nx, h->Ny, &h->fk));
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         h->fused_grid = sms > 0 ? sms : 148;
-        const size_t cps = (size_t)nz * (h->chi_has_v ? nv : 1);      // chi planes per slab
-        const size_t rcap = (size_t)2 << 30;                          // real-space chi kept per launch
-        size_t nss = rcap / (cps * rpp);
-        if (nss < 1) nss = 1;
-        if (nss > (size_t)nw * nspec) nss = (size_t)nw * nspec;
-        h->nss = (int)nss;
-        size_t nbz = ((size_t)64 << 20) / zpp;
-        if (nbz < 1) nbz = 1;
-        if (nbz > cps * nss) nbz = cps * nss;
-        h->nbz = (long long)nbz;
-        h->zbytes = zpp * nbz;
-        h->pbytes = 256;
-        h->rbytes = rpp * cps * nss;
     }
+    configure_batching(h);
 
     bool ok = upload_twiddles(h->Nx, &h->twx) && upload_twiddles(h->Ny, &h->twy) && alloc_scratch(h, &h->scr) &&
               (!h->em || cuda_ok(cudaMalloc(&h->vp_dev, sizeof(double) * (size_t)nv * nspec), "cudaMalloc(v_par)")) &&
@@ -564,34 +569,30 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
               (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
                                        : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
               upload_const_twiddles();
-    if (ok) {  // pipelined persistent x kernel (GENE_NL_PIPE=0: first-generation kernel)
-        const char* e = getenv("GENE_NL_PIPE");
-        // measured on B200: faster for Nx <= 192 (configs[4]: k_xinv 12.0 -> 10.2 ms), equal at 384, slower at 768
-        const int want = e ? atoi(e) : (h->Nx <= 192 ? 1 : 0);
+    if (ok && h->Nx <= 192) {
+        // pipelined persistent x kernel; measured on B200: faster for Nx <= 192 (configs[4]: k_xinv 12.0 -> 10.2 ms),
+        // equal at 384, slower at 768
         int sms = 0, occ = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if ((want & 1) && h->xk.smem_invp <= 227 * 1024 && set_smem(h->xk.invp, h->xk.smem_invp, "k_xinv_p smem") &&
+        if (h->xk.smem_invp <= 227 * 1024 && set_smem(h->xk.invp, h->xk.smem_invp, "k_xinv_p smem") &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
             h->xk.cap_invp = occ * sms;
     }
     if (ok && !h->chi_has_v && !h->em && !h->fused && (h->Nx / 2) % h->yk.rp_t == 0 && h->nky0 % h->xk.ck_zt == 0 &&
-        (h->Ny <= 192 || getenv("GENE_NL_ZT")) && h->yk.smem_t <= 227 * 1024 && h->xk.smem_invp_zt <= 227 * 1024) {
+        h->Ny <= 192 && h->yk.smem_t <= 227 * 1024 && h->xk.smem_invp_zt <= 227 * 1024) {
         // measured on B200: 384 x 192 (configs[2]) 7.79 -> 7.19 ms; at Ny = 384 the 105 KB of exchange tiles of
         // k_ybracket_t cost more than the stores save (configs[3]: 101 -> 119 ms), so that size keeps the row-major Z
-        const char* e = getenv("GENE_NL_ZT");  // development knob
         int sms = 0, occ = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if ((e ? atoi(e) : 1) && set_smem(h->yk.br_t, h->yk.smem_t, "k_ybracket_t smem") &&
+        if (set_smem(h->yk.br_t, h->yk.smem_t, "k_ybracket_t smem") &&
             set_smem(h->xk.invp_zt, h->xk.smem_invp_zt, "k_xinv_p<ZT> smem") &&
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp_zt, h->xk.nt, h->xk.smem_invp_zt) == cudaSuccess && occ > 0) {
             h->zt = true;
             h->cap_invp_zt = occ * sms;
         }
     }
-    if (ok && h->chi_has_v && !h->fused && (h->Nx / 2) % h->yk.rp_cv == 0 && h->yk.smem_cv <= 227 * 1024) {
-        const char* e = getenv("GENE_NL_NO_FUSE_CHI");  // development knob: k_yreal + R round trip instead
-        h->fuse_chi_y = !(e && atoi(e)) && set_smem(h->yk.br_cv, h->yk.smem_cv, "k_ybracket_cv smem");
-    }
+    if (ok && h->chi_has_v && !h->fused && (h->Nx / 2) % h->yk.rp_cv == 0 && h->yk.smem_cv <= 227 * 1024)
+        h->fuse_chi_y = set_smem(h->yk.br_cv, h->yk.smem_cv, "k_ybracket_cv smem");
     if (!ok) {
         std::string keep = g_err;
         gene_nl_destroy(h);
@@ -601,20 +602,70 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     return h;
 }
 
-void gene_nl_destroy(gene_nl_plan* h)
+static void free_stages(gene_nl_plan* h)
 {
-    if (!h) return;
-    cudaDeviceSynchronize();
     for (auto& s : h->stages) {
-        cudaFree(s.g); cudaFree(s.rhs); cudaFree(s.chi);
+        cudaFree(s.g); cudaFree(s.rhs); cudaFree(s.chi); cudaFree(s.apar);
         free_scratch(&s.scr);
         if (s.stream) cudaStreamDestroy(s.stream);
     }
+    h->stages.clear();
+}
+
+// The plan's tables, scratch and __constant__ twiddles live on the device it was created on
+static bool on_plan_device(const gene_nl_plan* h)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) {
+        set_err("the current CUDA device is not the one the plan was created on");
+        return false;
+    }
+    return true;
+}
+
+void gene_nl_destroy(gene_nl_plan* h)
+{
+    if (!h) return;
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != h->device) cudaSetDevice(h->device);  // free on the owning device, then restore
+    cudaDeviceSynchronize();
+    free_stages(h);
     free_scratch(&h->scr);
     cudaFree(h->twx);
     cudaFree(h->twy);
     cudaFree(h->vp_dev);
+    if (h->vp_pinned) cudaFreeHost(h->vp_pinned);
+    if (h->vp_event) cudaEventDestroy(h->vp_event);
+    if (cur >= 0 && cur != h->device) cudaSetDevice(cur);
     delete h;
+}
+
+int gene_nl_set_scratch_bytes(gene_nl_plan* h, size_t bytes)
+{
+    g_err.clear();
+    if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    if (bytes < ((size_t)1 << 20)) { set_err("gene_nl_set_scratch_bytes: the budget must be at least 1 MiB"); return GENE_NL_EINVAL; }
+    if (!on_plan_device(h)) return GENE_NL_EINVAL;
+    if (!cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize")) return GENE_NL_ECUDA;
+    const size_t old_budget = h->budget;
+    const bool old_set = h->budget_set;
+    free_stages(h);
+    free_scratch(&h->scr);
+    h->budget = bytes;
+    h->budget_set = true;
+    configure_batching(h);
+    if (!alloc_scratch(h, &h->scr)) {  // fall back to the previous budget so that the plan stays usable
+        std::string keep = g_err;
+        free_scratch(&h->scr);
+        h->budget = old_budget;
+        h->budget_set = old_set;
+        configure_batching(h);
+        if (!alloc_scratch(h, &h->scr)) { free_scratch(&h->scr); }
+        g_err = keep;
+        return GENE_NL_ENOMEM;
+    }
+    return GENE_NL_OK;
 }
 
 static int check_ptrs(const void* chi, const void* g, void* rhs, size_t gbytes, size_t cbytes)
@@ -633,6 +684,8 @@ static int compute_impl(gene_nl_plan* h, const void* chi_, const void* g_, void*
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
     if (h->em) { set_err("plan was created with GENE_NL_CHI_EM: call gene_nl_compute_em"); return GENE_NL_EINVAL; }
+    if (!on_plan_device(h)) return GENE_NL_EINVAL;
+    if (!h->scr.Z) { set_err("the plan has no scratch (an earlier gene_nl_set_scratch_bytes ran out of memory)"); return GENE_NL_ENOMEM; }
     const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
     const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
     int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
@@ -646,22 +699,41 @@ static int compute_impl(gene_nl_plan* h, const void* chi_, const void* g_, void*
     return GENE_NL_OK;
 }
 
-extern "C" int gene_nl_compute_em(gene_nl_plan* h, const void* phi_, const void* apar_, const double* vpar_host,
-                                  const void* g_, void* rhs_, double scale, void* stream)
+// em: v_par goes host -> plan-owned pinned staging -> device on `st`.  The staging buffer is reused by the next call,
+// so this one waits (on the host) for the previous call's copy; the caller's array is free when the call returns.
+static int stage_vpar(gene_nl_plan* h, const double* vpar_host, cudaStream_t st)
+{
+    const size_t n = (size_t)h->nv * h->nspec;
+    if (!h->vp_pinned) {
+        if (!cuda_ok(cudaMallocHost(&h->vp_pinned, sizeof(double) * n), "cudaMallocHost(v_par)")) return GENE_NL_ENOMEM;
+        if (!cuda_ok(cudaEventCreateWithFlags(&h->vp_event, cudaEventDisableTiming), "cudaEventCreate")) return GENE_NL_ECUDA;
+    } else if (!cuda_ok(cudaEventSynchronize(h->vp_event), "cudaEventSynchronize(v_par)")) {
+        return GENE_NL_ECUDA;
+    }
+    std::memcpy(h->vp_pinned, vpar_host, sizeof(double) * n);
+    if (!cuda_ok(cudaMemcpyAsync(h->vp_dev, h->vp_pinned, sizeof(double) * n, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync(v_par)") ||
+        !cuda_ok(cudaEventRecord(h->vp_event, st), "cudaEventRecord(v_par)"))
+        return GENE_NL_ECUDA;
+    return GENE_NL_OK;
+}
+
+int gene_nl_compute_em(gene_nl_plan* h, const void* phi_, const void* apar_, const double* vpar_host,
+                       const void* g_, void* rhs_, double scale, void* stream)
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
     if (!h->em) { set_err("gene_nl_compute_em needs a plan created with chi_has_v = GENE_NL_CHI_EM"); return GENE_NL_EINVAL; }
     if (!vpar_host) { set_err("NULL v_par array"); return GENE_NL_EINVAL; }
+    if (!on_plan_device(h)) return GENE_NL_EINVAL;
+    if (!h->scr.Z) { set_err("the plan has no scratch (an earlier gene_nl_set_scratch_bytes ran out of memory)"); return GENE_NL_ENOMEM; }
     const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
     const size_t cbytes = gbytes / h->nv;
     int rc = check_ptrs(phi_, g_, rhs_, gbytes, cbytes);
     if (!rc) rc = check_ptrs(apar_, g_, rhs_, gbytes, cbytes);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    if (!cuda_ok(cudaMemcpyAsync(h->vp_dev, vpar_host, sizeof(double) * (size_t)h->nv * h->nspec, cudaMemcpyHostToDevice, st),
-                 "cudaMemcpyAsync(v_par)"))
-        return GENE_NL_ECUDA;
+    rc = stage_vpar(h, vpar_host, st);
+    if (rc) return rc;
     if (enqueue_slabs(h, h->scr, (const cplx*)phi_, (const cplx*)g_, (cplx*)rhs_, h->nw * h->nspec, scale, st, nullptr,
                       (const cplx*)apar_) < 0)
         return GENE_NL_ECUDA;
@@ -694,45 +766,89 @@ int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, vo
     return cuda_ok(e, "cudaStreamSynchronize") ? GENE_NL_OK : GENE_NL_ECUDA;
 }
 
+// Host streaming: one chunk = one (w,s) slab = nz*nv contiguous planes of g and rhs and nz (or nz*nv)
+// planes of chi (em: nz planes of phi_bar and of A_par_bar); three stages, each with its own stream, staging buffers
+// and scratch set sized for ONE slab, so that the copies of one slab overlap the kernels of another.
+static int host_impl(gene_nl_plan* h, const void* chi_, const void* apar_, const void* g_, void* rhs_, double scale)
+{
+    const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
+    const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
+    int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
+    if (!rc && apar_) rc = check_ptrs(apar_, g_, rhs_, gbytes, cbytes);
+    if (rc) return rc;
+    const size_t slab_g = sizeof(cplx) * h->M * (size_t)h->nz * h->nv;
+    const size_t slab_c = h->chi_has_v ? slab_g : slab_g / h->nv;
+    if (h->stages.empty()) {
+        // built locally and moved into the plan only when every allocation succeeded
+        const int nstage = 3;
+        std::vector<HostStage> st(nstage);
+        size_t rbytes1 = h->rbytes;  // a stage's scratch set serves one slab
+        if (h->fused) rbytes1 = sizeof(cplx) * (size_t)h->Nx * h->Ny * (size_t)h->nz * (h->chi_has_v ? h->nv : 1);
+        bool ok = true;
+        for (auto& s : st) {
+            ok = ok && cuda_ok(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate") &&
+                 cuda_ok(cudaMalloc(&s.g, slab_g), "cudaMalloc(stage g)") &&
+                 cuda_ok(cudaMalloc(&s.rhs, slab_g), "cudaMalloc(stage rhs)") &&
+                 cuda_ok(cudaMalloc(&s.chi, slab_c), "cudaMalloc(stage chi)") &&
+                 (!h->em || cuda_ok(cudaMalloc(&s.apar, slab_c), "cudaMalloc(stage A_par)")) &&
+                 alloc_scratch(h->zbytes, h->pbytes, rbytes1, &s.scr);
+            if (!ok) break;
+        }
+        if (!ok) {
+            std::string keep = g_err;
+            for (auto& s : st) {
+                cudaFree(s.g); cudaFree(s.rhs); cudaFree(s.chi); cudaFree(s.apar);
+                free_scratch(&s.scr);
+                if (s.stream) cudaStreamDestroy(s.stream);
+            }
+            g_err = keep;
+            return GENE_NL_ENOMEM;
+        }
+        h->stages = std::move(st);
+    }
+    const char* chi = (const char*)chi_;
+    const char* apar = (const char*)apar_;
+    const char* g = (const char*)g_;
+    char* rhs = (char*)rhs_;
+    int ret = GENE_NL_OK;
+    for (int ws = 0; ws < h->nw * h->nspec && ret == GENE_NL_OK; ++ws) {
+        HostStage& s = h->stages[ws % h->stages.size()];
+        bool ok = cuda_ok(cudaMemcpyAsync(s.g, g + ws * slab_g, slab_g, cudaMemcpyHostToDevice, s.stream), "H2D g") &&
+                  cuda_ok(cudaMemcpyAsync(s.rhs, rhs + ws * slab_g, slab_g, cudaMemcpyHostToDevice, s.stream), "H2D rhs") &&
+                  cuda_ok(cudaMemcpyAsync(s.chi, chi + ws * slab_c, slab_c, cudaMemcpyHostToDevice, s.stream), "H2D chi") &&
+                  (!apar || cuda_ok(cudaMemcpyAsync(s.apar, apar + ws * slab_c, slab_c, cudaMemcpyHostToDevice, s.stream), "H2D A_par"));
+        if (!ok) { ret = GENE_NL_ECUDA; break; }
+        if (enqueue_slabs(h, s.scr, s.chi, s.g, s.rhs, 1, scale, s.stream, nullptr, apar ? s.apar : nullptr, ws) < 0) { ret = GENE_NL_ECUDA; break; }
+        if (!cuda_ok(cudaMemcpyAsync(rhs + ws * slab_g, s.rhs, slab_g, cudaMemcpyDeviceToHost, s.stream), "D2H rhs")) ret = GENE_NL_ECUDA;
+    }
+    for (auto& s : h->stages)
+        if (!cuda_ok(cudaStreamSynchronize(s.stream), "cudaStreamSynchronize") && ret == GENE_NL_OK) ret = GENE_NL_ECUDA;
+    return ret;
+}
+
 int gene_nl_compute_host(gene_nl_plan* h, const void* chi_, const void* g_, void* rhs_, double scale)
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
-    if (h->em) { set_err("gene_nl_compute_host: not available for GENE_NL_CHI_EM plans"); return GENE_NL_EINVAL; }
-    const size_t gbytes = sizeof(cplx) * h->M * (size_t)h->planes;
-    const size_t cbytes = h->chi_has_v ? gbytes : gbytes / h->nv;
-    int rc = check_ptrs(chi_, g_, rhs_, gbytes, cbytes);
+    if (h->em) { set_err("plan was created with GENE_NL_CHI_EM: call gene_nl_compute_em_host"); return GENE_NL_EINVAL; }
+    if (!on_plan_device(h)) return GENE_NL_EINVAL;
+    return host_impl(h, chi_, nullptr, g_, rhs_, scale);
+}
+
+int gene_nl_compute_em_host(gene_nl_plan* h, const void* phi_, const void* apar_, const double* vpar_host, const void* g_,
+                            void* rhs_, double scale)
+{
+    g_err.clear();
+    if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    if (!h->em) { set_err("gene_nl_compute_em_host needs a plan created with chi_has_v = GENE_NL_CHI_EM"); return GENE_NL_EINVAL; }
+    if (!vpar_host || !apar_) { set_err("NULL v_par or A_par array"); return GENE_NL_EINVAL; }
+    if (!on_plan_device(h)) return GENE_NL_EINVAL;
+    // v_par reaches the device before any stage starts (legacy default stream + a device-wide wait is simplest and
+    // happens once per call)
+    int rc = stage_vpar(h, vpar_host, nullptr);
     if (rc) return rc;
-    // one chunk = one (w,s) slab: nz*nv contiguous planes of g and rhs, nz (or nz*nv) planes of chi
-    const size_t slab_g = sizeof(cplx) * h->M * (size_t)h->nz * h->nv;
-    const size_t slab_c = h->chi_has_v ? slab_g : slab_g / h->nv;
-    if (h->stages.empty()) {
-        const int nstage = 3;
-        h->stages.resize(nstage);
-        for (auto& s : h->stages) {
-            bool ok = cuda_ok(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate") &&
-                      cuda_ok(cudaMalloc(&s.g, slab_g), "cudaMalloc(stage g)") &&
-                      cuda_ok(cudaMalloc(&s.rhs, slab_g), "cudaMalloc(stage rhs)") &&
-                      cuda_ok(cudaMalloc(&s.chi, slab_c), "cudaMalloc(stage chi)") && alloc_scratch(h, &s.scr);
-            if (!ok) return GENE_NL_ENOMEM;
-        }
-    }
-    const char* chi = (const char*)chi_;
-    const char* g = (const char*)g_;
-    char* rhs = (char*)rhs_;
-    for (int ws = 0; ws < h->nw * h->nspec; ++ws) {
-        HostStage& s = h->stages[ws % h->stages.size()];
-        bool ok = cuda_ok(cudaMemcpyAsync(s.g, g + ws * slab_g, slab_g, cudaMemcpyHostToDevice, s.stream), "H2D g") &&
-                  cuda_ok(cudaMemcpyAsync(s.rhs, rhs + ws * slab_g, slab_g, cudaMemcpyHostToDevice, s.stream), "H2D rhs") &&
-                  cuda_ok(cudaMemcpyAsync(s.chi, chi + ws * slab_c, slab_c, cudaMemcpyHostToDevice, s.stream), "H2D chi");
-        if (!ok) return GENE_NL_ECUDA;
-        if (enqueue_slabs(h, s.scr, s.chi, s.g, s.rhs, 1, scale, s.stream) < 0) return GENE_NL_ECUDA;
-        if (!cuda_ok(cudaMemcpyAsync(rhs + ws * slab_g, s.rhs, slab_g, cudaMemcpyDeviceToHost, s.stream), "D2H rhs"))
-            return GENE_NL_ECUDA;
-    }
-    for (auto& s : h->stages)
-        if (!cuda_ok(cudaStreamSynchronize(s.stream), "cudaStreamSynchronize")) return GENE_NL_ECUDA;
-    return GENE_NL_OK;
+    if (!cuda_ok(cudaEventSynchronize(h->vp_event), "cudaEventSynchronize(v_par)")) return GENE_NL_ECUDA;
+    return host_impl(h, phi_, apar_, g_, rhs_, scale);
 }
 
 size_t gene_nl_workspace_bytes(const gene_nl_plan* h)

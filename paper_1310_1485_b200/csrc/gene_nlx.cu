@@ -55,12 +55,21 @@ bool ok_or_err(cudaError_t e, const char* what)
 
 }  // namespace
 
+struct XgStage {  // per-stream staging of one chunk of planes for gene_nlx_compute_host
+    cudaStream_t stream = nullptr;
+    cplx* buf[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};  // vex, vey, dxg, dyg, rhs
+};
+
 struct gene_nlx_plan {
     int nx, nky0, Ny;
     long long planes;
     XgKernel k;
     cplx* tw = nullptr;
     int grid_cap = 0;
+    int device = -1;
+    std::vector<XgStage> stages;  // lazily created by gene_nlx_compute_host
+    long long chunk = 0;          // planes per chunk
+    double* pref_dev = nullptr;
 };
 
 extern "C" {
@@ -75,7 +84,7 @@ gene_nlx_plan* gene_nlx_create(int nx, int nky0, long long planes)
     int dev = -1;
     if (!ok_or_err(cudaGetDevice(&dev), "cudaGetDevice (no CUDA device: this library has no CPU fallback)")) return nullptr;
     gene_nlx_plan* h = new gene_nlx_plan();
-    h->nx = nx; h->nky0 = nky0; h->Ny = 3 * nky0; h->planes = planes;
+    h->nx = nx; h->nky0 = nky0; h->Ny = 3 * nky0; h->planes = planes; h->device = dev;
     if (!find_xg(h->Ny, &h->k)) {
         gene_nl_set_error_("gene_nlx_create: unsupported nky0 (padded y grid Ny = 3 nky0 must be 24, 48 or 96)");
         delete h;
@@ -103,11 +112,15 @@ gene_nlx_plan* gene_nlx_create(int nx, int nky0, long long planes)
     return h;
 }
 
-int gene_nlx_compute(gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
-                     const double* pref, void* rhs, double scale, void* stream)
+static int check_args(const gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
+                      const double* pref, const void* rhs)
 {
-    gene_nl_set_error_("");
     if (!h) { gene_nl_set_error_("NULL plan"); return GENE_NL_EINVAL; }
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) {
+        gene_nl_set_error_("the current CUDA device is not the one the plan was created on");
+        return GENE_NL_EINVAL;
+    }
     if (!vex || !vey || !dxg || !dyg || !pref || !rhs) { gene_nl_set_error_("NULL array pointer"); return GENE_NL_EINVAL; }
     if (((uintptr_t)vex | (uintptr_t)vey | (uintptr_t)dxg | (uintptr_t)dyg | (uintptr_t)rhs) & 15) {
         gene_nl_set_error_("array pointers must be 16-byte aligned");
@@ -119,20 +132,95 @@ int gene_nlx_compute(gene_nlx_plan* h, const void* vex, const void* vey, const v
         const char* a = (const char*)in;
         if (a < r0 + bytes && r0 < a + bytes) { gene_nl_set_error_("rhs overlaps an input array"); return GENE_NL_EINVAL; }
     }
+    return GENE_NL_OK;
+}
+
+// one launch of k_xglobal over `planes` planes starting at the given device pointers
+static bool launch(const gene_nlx_plan* h, const cplx* vex, const cplx* vey, const cplx* dxg, const cplx* dyg,
+                   const double* pref, cplx* rhs, long long planes, double scale, cudaStream_t st)
+{
     const int xtiles = (h->nx + h->k.xt - 1) / h->k.xt;
-    const long long ntiles = h->planes * xtiles;
+    const long long ntiles = planes * xtiles;
     const int grid = (int)(ntiles < h->grid_cap ? ntiles : h->grid_cap);
     const double coef = scale / (2.0 * (double)h->Ny);
-    h->k.fn<<<grid, h->k.nt, h->k.smem, (cudaStream_t)stream>>>((const cplx*)vex, (const cplx*)vey, (const cplx*)dxg,
-                                                               (const cplx*)dyg, pref, (cplx*)rhs, h->tw, h->nx, xtiles,
-                                                               ntiles, coef);
-    return ok_or_err(cudaGetLastError(), "k_xglobal launch") ? GENE_NL_OK : GENE_NL_ECUDA;
+    h->k.fn<<<grid, h->k.nt, h->k.smem, st>>>(vex, vey, dxg, dyg, pref, rhs, h->tw, h->nx, xtiles, ntiles, coef);
+    return ok_or_err(cudaGetLastError(), "k_xglobal launch");
+}
+
+int gene_nlx_compute(gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
+                     const double* pref, void* rhs, double scale, void* stream)
+{
+    gene_nl_set_error_("");
+    const int rc = check_args(h, vex, vey, dxg, dyg, pref, rhs);
+    if (rc) return rc;
+    return launch(h, (const cplx*)vex, (const cplx*)vey, (const cplx*)dxg, (const cplx*)dyg, pref, (cplx*)rhs, h->planes,
+                  scale, (cudaStream_t)stream) ? GENE_NL_OK : GENE_NL_ECUDA;
+}
+
+static void free_xg_stages(gene_nlx_plan* h)
+{
+    for (auto& s : h->stages) {
+        for (cplx* b : s.buf) cudaFree(b);
+        if (s.stream) cudaStreamDestroy(s.stream);
+    }
+    h->stages.clear();
+    cudaFree(h->pref_dev);
+    h->pref_dev = nullptr;
+}
+
+// "we split each input array into (usually four) contiguous chunks of xy-planes, which are transferred
+// and computed in two asynchronous CUDA streams".  Here: chunks of <= 64 MiB per array (at least four per call when
+// the arrays allow it), three streams, so that the H2D copies of one chunk, the kernel of another and the D2H copy of
+// a third overlap; 5 planes go in and 1 comes out per plane computed.
+int gene_nlx_compute_host(gene_nlx_plan* h, const void* vex, const void* vey, const void* dxg, const void* dyg,
+                          const double* pref, void* rhs, double scale)
+{
+    gene_nl_set_error_("");
+    const int rc = check_args(h, vex, vey, dxg, dyg, pref, rhs);
+    if (rc) return rc;
+    const size_t plane_bytes = sizeof(cplx) * (size_t)h->nx * h->nky0;
+    if (h->stages.empty()) {
+        long long chunk = (long long)(((size_t)64 << 20) / plane_bytes);
+        if (chunk > (h->planes + 3) / 4) chunk = (h->planes + 3) / 4;
+        if (chunk < 1) chunk = 1;
+        std::vector<XgStage> st(3);
+        bool ok = ok_or_err(cudaMalloc(&h->pref_dev, sizeof(double) * h->nx), "cudaMalloc(pref)");
+        for (auto& s : st) {
+            ok = ok && ok_or_err(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate");
+            for (auto& b : s.buf) ok = ok && ok_or_err(cudaMalloc(&b, plane_bytes * (size_t)chunk), "cudaMalloc(stage)");
+            if (!ok) break;
+        }
+        h->stages = std::move(st);
+        if (!ok) { free_xg_stages(h); return GENE_NL_ENOMEM; }
+        h->chunk = chunk;
+    }
+    if (!ok_or_err(cudaMemcpy(h->pref_dev, pref, sizeof(double) * h->nx, cudaMemcpyHostToDevice), "cudaMemcpy(pref)"))
+        return GENE_NL_ECUDA;
+    const char* in[4] = {(const char*)vex, (const char*)vey, (const char*)dxg, (const char*)dyg};
+    char* out = (char*)rhs;
+    int ret = GENE_NL_OK;
+    long long c = 0;
+    for (long long p0 = 0; p0 < h->planes && ret == GENE_NL_OK; p0 += h->chunk, ++c) {
+        XgStage& s = h->stages[c % h->stages.size()];
+        const long long np = (h->planes - p0 < h->chunk) ? h->planes - p0 : h->chunk;
+        const size_t off = plane_bytes * (size_t)p0, nb = plane_bytes * (size_t)np;
+        bool ok = true;
+        for (int a = 0; a < 4; ++a) ok = ok && ok_or_err(cudaMemcpyAsync(s.buf[a], in[a] + off, nb, cudaMemcpyHostToDevice, s.stream), "H2D");
+        ok = ok && ok_or_err(cudaMemcpyAsync(s.buf[4], out + off, nb, cudaMemcpyHostToDevice, s.stream), "H2D rhs") &&
+             launch(h, s.buf[0], s.buf[1], s.buf[2], s.buf[3], h->pref_dev, s.buf[4], np, scale, s.stream) &&
+             ok_or_err(cudaMemcpyAsync(out + off, s.buf[4], nb, cudaMemcpyDeviceToHost, s.stream), "D2H rhs");
+        if (!ok) ret = GENE_NL_ECUDA;
+    }
+    for (auto& s : h->stages)
+        if (!ok_or_err(cudaStreamSynchronize(s.stream), "cudaStreamSynchronize") && ret == GENE_NL_OK) ret = GENE_NL_ECUDA;
+    return ret;
 }
 
 void gene_nlx_destroy(gene_nlx_plan* h)
 {
     if (!h) return;
     cudaDeviceSynchronize();
+    free_xg_stages(h);
     cudaFree(h->tw);
     delete h;
 }

@@ -1,10 +1,10 @@
 // probe.cu -- micro-benchmarks of the two units that bound the FFT path on one SM: the FP64 FMA pipe
 // and the shared-memory crossbar ("FP64 37.2 TFLOP/s is a model ... first GPU task: a
 // DFMA-chain microbenchmark (and a 128-bit SMEM ld/st bandwidth one)").  Exported as
-// gene_nl_probe_peaks (include/gene_nl.h); bench.py uses it for the roofline denominators.
+// gene_nl_probe_peaks (include/gene_nl_bench.h); bench.py uses it for the roofline denominators.
 #include <cuda_runtime.h>
 
-#include "../../include/gene_nl.h"
+#include "../../include/gene_nl_bench.h"
 
 namespace {
 

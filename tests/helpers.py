@@ -11,7 +11,10 @@ TOL = 1e-11  # north_star: max over planes of ||N_gpu - N_ref||_2 / ||N_ref||_2 
 
 
 def sample_planes(wl, n, seed=0):
-    """First/last plane, first/last index of each of z, v, w, s, plus seeded random planes."""
+    """Planes to compare when the oracle cannot do them all.  Never truncated: always planes 0 and P-1 and the 16
+    corners (first/last index of each of z, v, w, s: both species, first and last slab), then one seeded random plane in
+    EVERY (w,s) slab (a wrong plane -> CTA map or a ragged batch tail shows up inside slabs, not only at the ends), then
+    seeded random planes until at least max(n, corners + slabs + 32) planes are picked."""
     P = wl.planes
     picks = {0, P - 1}
     for z in (0, wl.nz - 1):
@@ -20,9 +23,13 @@ def sample_planes(wl, n, seed=0):
                 for s in (0, wl.nspec - 1):
                     picks.add(z + wl.nz * (v + wl.nv * (w + wl.nw * s)))
     rng = np.random.default_rng(seed)
-    while len(picks) < min(n, P):
+    per_slab = wl.nz * wl.nv
+    for ws in range(wl.nw * wl.nspec):
+        picks.add(ws * per_slab + int(rng.integers(0, per_slab)))
+    want = min(P, max(n, len(picks) + 32))
+    while len(picks) < want:
         picks.add(int(rng.integers(0, P)))
-    return np.array(sorted(picks)[:max(n, 2)] if len(picks) > n else sorted(picks))
+    return np.array(sorted(picks))
 
 
 def oracle_on_planes(wl, chi, g, rhs_in, planes, scale=None, backend=oracle.DFT_RECURSIVE):
@@ -45,11 +52,20 @@ def plane_errors(wl, out_planes, ref, R_in):
     return num / den
 
 
-def gpu_compute(wl, chi, g, rhs, scale=None, host=False):
+def plane_max_errors(wl, out_planes, ref, R_in):
+    """Element-wise companion of the R14 norm: per plane max |rhs_gpu - rhs_ref| / max |scale N_ref|.  The L2 norm over
+    a 65 536-mode plane hides one wrong mode at 1e-9; this bound (same 1e-11) does not."""
+    num = np.abs(out_planes - ref).reshape(len(ref), -1).max(axis=1)
+    den = np.abs(ref - R_in).reshape(len(ref), -1).max(axis=1)
+    assert np.all(den > 0)
+    return num / den
+
+
+def gpu_compute(wl, chi, g, rhs, scale=None, host=False, scratch_bytes=None):
     """rhs += scale*N through the C ABI; returns the updated rhs tensor (a new tensor)."""
     from paper_1310_1485_b200 import GeneNL
     out = rhs.clone()
-    with GeneNL(wl) as nl:
+    with GeneNL(wl, scratch_bytes=scratch_bytes) as nl:
         if host:
             nl.compute_host(chi, g, out, scale)
         else:
@@ -58,17 +74,23 @@ def gpu_compute(wl, chi, g, rhs, scale=None, host=False):
     return out
 
 
-def check_parity(wl, device, nsample=None, host=False, tol=TOL, backend=oracle.DFT_RECURSIVE):
+def check_parity(wl, device, nsample=None, host=False, tol=TOL, backend=oracle.DFT_RECURSIVE, scratch_bytes=None):
     chi, g, rhs = W.make_inputs(wl, device if not host else "cpu")
     if host:
         chi, g, rhs = chi.pin_memory(), g.pin_memory(), rhs.pin_memory()
-    out = gpu_compute(wl, chi, g, rhs, host=host)
+    out = gpu_compute(wl, chi, g, rhs, host=host, scratch_bytes=scratch_bytes)
     planes = np.arange(wl.planes) if nsample is None or nsample >= wl.planes else sample_planes(wl, nsample, wl.seed)
-    ref, R, _, _ = oracle_on_planes(wl, chi, g, rhs, planes, backend=backend)
-    idx = torch.as_tensor(planes, dtype=torch.long, device=out.device)
-    got = W.as_planes(out, wl)[idx].cpu().numpy()
-    err = plane_errors(wl, got, ref, R)
+    err, emax = [], []
+    for c0 in range(0, len(planes), 1024):   # the oracle in bounded chunks (host memory)
+        sel = planes[c0:c0 + 1024]
+        ref, R, _, _ = oracle_on_planes(wl, chi, g, rhs, sel, backend=backend)
+        idx = torch.as_tensor(sel, dtype=torch.long, device=out.device)
+        got = W.as_planes(out, wl)[idx].cpu().numpy()
+        err.append(plane_errors(wl, got, ref, R))
+        emax.append(plane_max_errors(wl, got, ref, R))
+    err, emax = np.concatenate(err), np.concatenate(emax)
     assert err.max() <= tol, f"{wl.name}: max plane error {err.max():.3e} at plane {planes[err.argmax()]}"
+    assert emax.max() <= tol, f"{wl.name}: max element error {emax.max():.3e} at plane {planes[emax.argmax()]}"
     # Nyquist row of rhs untouched, bit for bit (R6)
     h = wl.nx0 // 2
     assert torch.equal(W.as_planes(out, wl)[:, :, h], W.as_planes(rhs, wl)[:, :, h])

@@ -9,8 +9,8 @@ import pytest
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_functions():
-    src = open(os.path.join(ROOT, "include", "gene_nl.h")).read()
+def declared_functions(header="gene_nl.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(gene_nlx?_\w+)\s*\(", src)))
 
@@ -28,6 +28,9 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     assert os.path.dirname(binding.library_path()) == os.path.join(ROOT, "paper_1310_1485_b200")
     names = declared_functions()
     assert sorted(binding.EXPORTED_SYMBOLS) == names
+    bench_names = declared_functions("gene_nl_bench.h")          # benchmark-only helpers, in a header of their own
+    assert sorted(binding.BENCH_SYMBOLS) == bench_names and not set(bench_names) & set(names)
+    names = names + bench_names
     for n in names:
         assert hasattr(lib, n), n
     raw = ctypes.CDLL(binding.library_path())
@@ -51,6 +54,18 @@ def test_no_cpu_fallback_without_a_device():
     from paper_1310_1485_b200 import gene_nlx_create
     with pytest.raises(GeneNLError):
         gene_nlx_create(64, 16, 1)
+
+
+def test_no_environment_knobs_in_the_product_path():
+    """SURVEY.md sect. 5: configuration comes through gene_nl_create arguments only (no env flags)."""
+    pkg = os.path.join(ROOT, "paper_1310_1485_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "getenv" not in text, f
+                if f != "build.py":   # build.py may honour NVCC (the compiler's location), nothing else
+                    assert "os.environ" not in text, f
 
 
 def test_product_path_does_not_touch_the_oracle():

@@ -37,20 +37,30 @@ def composed_chi(wl, phi, apar, vpar):
     return chi
 
 
-def run_em(wl, phi, apar, vpar, g, rhs):
-    from paper_1310_1485_b200 import GENE_NL_CHI_EM, gene_nl_compute_em, gene_nl_create, gene_nl_destroy
+def run_em(wl, phi, apar, vpar, g, rhs, scratch_bytes=None, host=False):
+    from paper_1310_1485_b200 import (GENE_NL_CHI_EM, gene_nl_compute_em, gene_nl_compute_em_host, gene_nl_create,
+                                      gene_nl_destroy, gene_nl_set_scratch_bytes)
     out = rhs.clone()
     h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
     try:
-        gene_nl_compute_em(h, phi, apar, vpar, g, out, wl.scale)
-        torch.cuda.synchronize()
+        if scratch_bytes is not None:
+            gene_nl_set_scratch_bytes(h, scratch_bytes)
+        if host:
+            hp, ha, hg, ho = (t.cpu().pin_memory() for t in (phi, apar, g, out))
+            gene_nl_compute_em_host(h, hp, ha, vpar, hg, ho, wl.scale)
+            out = ho.to(rhs.device)
+        else:
+            gene_nl_compute_em(h, phi, apar, vpar, g, out, wl.scale)
+            gene_nl_compute_em(h, phi, apar, 0.0 * vpar, g, out, 0.0)   # a second call reuses the v_par staging buffer
+            torch.cuda.synchronize()
     finally:
         gene_nl_destroy(h)
     return out
 
 
 SHAPES = [(16, 8, 3, 5, 2, 2), (64, 32, 2, 3, 2, 1), (96, 48, 2, 4, 1, 2), (128, 32, 3, 3, 1, 1), (256, 64, 2, 2, 1, 2),
-          (32, 128, 1, 3, 1, 1)]
+          (32, 128, 1, 3, 1, 1),
+          (256, 64, 36, 2, 1, 1)]   # chi rows of a chunk beyond 40 MB: k_ybracket<EM> walks its tiles v-fastest
 
 
 @pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec", SHAPES)
@@ -64,12 +74,11 @@ def test_em_matches_oracle_on_composed_chi(cuda_device, nx0, nky0, nz, nv, nw, n
     assert plane_errors(wl, W.as_planes(out, wl).cpu().numpy(), ref, R).max() <= TOL
 
 
-def test_em_under_a_tiny_scratch_budget_and_against_the_per_plane_chi_path(cuda_device, monkeypatch):
+def test_em_under_a_tiny_scratch_budget_and_against_the_per_plane_chi_path(cuda_device):
     from helpers import gpu_compute
-    monkeypatch.setenv("GENE_NL_SCRATCH_MB", "2")
     wl = W.small_workload(64, 32, 5, 7, 2, 2, 0.05, 0.05, False, seed=31)
     phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
-    out = run_em(wl, phi, apar, vpar, g, rhs)
+    out = run_em(wl, phi, apar, vpar, g, rhs, scratch_bytes=2 << 20)
     chi = composed_chi(wl, phi, apar, vpar)
     G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
     ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
@@ -80,6 +89,20 @@ def test_em_under_a_tiny_scratch_budget_and_against_the_per_plane_chi_path(cuda_
     out_v = gpu_compute(wlv, chi_t, g, rhs)
     d = (out - out_v).abs().max().item()
     assert d <= 1e-12 * (out_v - rhs).abs().max().item()
+
+
+def test_em_host_entry_point_matches_the_device_entry_point(cuda_device):
+    """gene_nl_compute_em_host streams (w,s) slabs through the same kernels: the same bits as gene_nl_compute_em; the
+    species index of a slab (v_par is per species) must survive the slab-by-slab walk."""
+    wl = W.small_workload(64, 32, 3, 4, 3, 2, 0.05, 0.05, False, seed=33)
+    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+    dev = run_em(wl, phi, apar, vpar, g, rhs)
+    hst = run_em(wl, phi, apar, vpar, g, rhs, host=True)
+    assert torch.equal(dev, hst)
+    chi = composed_chi(wl, phi, apar, vpar)
+    G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
+    ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
+    assert plane_errors(wl, W.as_planes(hst, wl).cpu().numpy(), ref, R).max() <= TOL
 
 
 def test_em_errors(cuda_device):

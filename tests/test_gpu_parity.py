@@ -13,11 +13,6 @@ from paper_1310_1485_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(autouse=True)
-def _default_budget(monkeypatch):
-    monkeypatch.delenv("GENE_NL_SCRATCH_MB", raising=False)
-
-
 def test_config0_all_planes_against_oracle_and_definition(cuda_device):
     wl = W.CONFIGS[0]
     err = check_parity(wl, cuda_device, backend=oracle.DFT_NAIVE)
@@ -41,6 +36,10 @@ SHAPES = [
     (256, 64, 2, 2, 1, 1, False), (32, 128, 1, 3, 1, 1, False),
     (512, 16, 1, 2, 1, 1, True), (16, 8, 1, 1, 1, 1, False),
     (256, 64, 36, 2, 1, 1, False),   # chi rows of a chunk beyond 40 MB: the v-fastest tile walk of k_ybracket_t
+    # Nx = 768 with chi shared over v and Ny <= 192: k_xinv_p<768,...,ZT> + k_ybracket_t (on by default at these sizes)
+    (512, 16, 2, 3, 1, 1, False), (512, 64, 1, 2, 1, 1, False),
+    (512, 128, 1, 2, 1, 1, False),   # the plane shape of configs[3]: k_xinv<768,...,SEQ> + k_ybracket<384> + k_xfwd<768>
+    (512, 128, 1, 1, 1, 1, True),
 ]
 
 
@@ -50,12 +49,33 @@ def test_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, nw, nspec, chi_
     check_parity(wl, cuda_device)
 
 
-@pytest.mark.parametrize("budget_mb", ["1", "3"])
-def test_ragged_batches_under_a_tiny_scratch_budget(cuda_device, monkeypatch, budget_mb):
-    monkeypatch.setenv("GENE_NL_SCRATCH_MB", budget_mb)
-    for chi_has_v in (False, True):
-        wl = W.small_workload(64, 32, 5, 7, 2, 1, 0.05, 0.05, chi_has_v, seed=21)
-        check_parity(wl, cuda_device)
+@pytest.mark.parametrize("budget_mb", [1, 3])
+def test_ragged_batches_under_a_tiny_scratch_budget(cuda_device, budget_mb):
+    """gene_nl_set_scratch_bytes: more and smaller batches (ragged z and v tails), never a different result.
+    64 x 32 planes take the fused kernel (the budget bounds its chi cache: several launches), 64 x 64 the batched ones."""
+    for nky0 in (32, 64):
+        for chi_has_v in (False, True):
+            wl = W.small_workload(64, nky0, 5, 7, 2, 1, 0.05, 0.05, chi_has_v, seed=21)
+            check_parity(wl, cuda_device, scratch_bytes=budget_mb << 20)
+
+
+def test_set_scratch_bytes_changes_the_batching_not_the_bits(cuda_device):
+    from paper_1310_1485_b200 import GeneNL, GeneNLError, gene_nl_set_scratch_bytes
+    wl = W.small_workload(64, 64, 5, 7, 2, 1, 0.05, 0.05, False, seed=23)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    base = gpu_compute(wl, chi, g, rhs)
+    with GeneNL(wl) as nl:
+        n0 = nl.launches_per_compute
+        gene_nl_set_scratch_bytes(nl.h, 2 << 20)
+        assert nl.launches_per_compute > n0
+        out = rhs.clone()
+        nl.compute(chi, g, out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, base)                 # planes are independent: the same bits whatever the batching
+        with pytest.raises(GeneNLError):
+            gene_nl_set_scratch_bytes(nl.h, 1000)      # below 1 MiB
+        nl.compute(chi, g, out)                        # the plan still works afterwards
+        torch.cuda.synchronize()
 
 
 def test_properties_scale_zero_linearity_antisymmetry(cuda_device):
@@ -97,12 +117,12 @@ def test_non_hermitian_ky0_column_follows_reading_R7(cuda_device):
     assert plane_errors(wl, W.as_planes(out, wl).cpu().numpy(), ref, R).max() <= TOL
 
 
-def test_host_entry_point_matches_oracle(cuda_device, monkeypatch):
+def test_host_entry_point_matches_oracle(cuda_device):
     check_parity(W.CONFIGS[0], cuda_device, host=True)
-    monkeypatch.setenv("GENE_NL_SCRATCH_MB", "2")
-    for chi_has_v in (False, True):
-        wl = W.small_workload(64, 32, 5, 3, 2, 2, 0.05, 0.05, chi_has_v, seed=22)
-        check_parity(wl, cuda_device, host=True)
+    for nky0 in (32, 64):           # fused and batched kernels behind the streaming driver
+        for chi_has_v in (False, True):
+            wl = W.small_workload(64, nky0, 5, 3, 2, 2, 0.05, 0.05, chi_has_v, seed=22)
+            check_parity(wl, cuda_device, host=True, scratch_bytes=2 << 20)
 
 
 def test_errors_are_reported_not_swallowed(cuda_device):
@@ -137,20 +157,37 @@ def _full_size(cuda_device, idx, nsample):
     return check_parity(wl, cuda_device, nsample=nsample)
 
 
-def test_config1_full_size_sampled_planes(cuda_device):
-    _full_size(cuda_device, 1, 48)
+def test_config1_full_size_all_planes(cuda_device):
+    _full_size(cuda_device, 1, None)       # all 8192 planes (the oracle needs ~5 s on 16 cores)
 
 
-def test_config2_full_size_sampled_planes(cuda_device):
-    _full_size(cuda_device, 2, 20)
+def test_config2_full_size_all_planes(cuda_device):
+    _full_size(cuda_device, 2, None)       # all 8192 planes (~25 s)
 
 
 def test_config4_full_size_sampled_planes(cuda_device):
-    _full_size(cuda_device, 4, 24)
+    _full_size(cuda_device, 4, 160)        # corners, one random plane in each of the 48 (w,s) slabs, random planes
 
 
 def test_config3_full_size_sampled_planes(cuda_device):
-    _full_size(cuda_device, 3, 6)
+    _full_size(cuda_device, 3, 96)         # corners, one random plane in each of the 32 (w,s) slabs, random planes
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_plane_sharded_ranks_assemble_to_the_unsharded_result(cuda_device, world):
+    """planes are independent given chi, so (w,s) slabs shard over ranks with no
+    exchange.  One GPU here: each rank's shard (workloads.shard_arrays) goes through gene_nl_compute in turn and the
+    assembled rhs must equal the unsharded call bit for bit; batched and fused kernels, chi with and without v."""
+    for nx0, nky0, chi_has_v in ((64, 64, False), (128, 32, False), (64, 64, True)):
+        wl = W.small_workload(nx0, nky0, 3, 4, 5, 1, 0.05, 0.05, chi_has_v, seed=50 + world)
+        chi, g, rhs = W.make_inputs(wl, cuda_device)
+        whole = gpu_compute(wl, chi, g, rhs)
+        parts = []
+        for rank in range(world):
+            sub, cs, gs, rs = W.shard_arrays(wl, chi, g, rhs, rank, world)
+            assert sub.nw >= 1
+            parts.append(gpu_compute(sub, cs.contiguous(), gs.contiguous(), rs.contiguous()).reshape(-1))
+        assert torch.equal(torch.cat(parts), whole.reshape(-1))
 
 
 def test_config1_sampled_modes_against_the_definition(cuda_device):

@@ -74,6 +74,25 @@ def test_paper_shape_sampled_planes(cuda_device):
     assert plane_errors(wl, arrs, out, planes).max() <= TOL
 
 
+def test_host_entry_point_streams_chunks_to_the_same_bits(cuda_device):
+    """gene_nlx_compute_host (chunks of xy-planes on asynchronous streams): same kernel per chunk, so the
+    same bits as the device-resident call; 37 planes = 4 ragged chunks, and enough planes for several 64 MiB chunks."""
+    from paper_1310_1485_b200 import gene_nlx_compute_host, gene_nlx_create, gene_nlx_destroy
+    for planes in (37, 20000):
+        wl = W.XGlobalWorkload("xg_host", 64, 16, planes, 12, 0.7)
+        arrs = W.make_xglobal_inputs(wl, cuda_device)
+        dev = run_gpu(wl, arrs)
+        vex, vey, dxg, dyg, pref, rhs = (t.cpu().pin_memory() for t in arrs)
+        h = gene_nlx_create(wl.nx, wl.nky0, wl.planes)
+        try:
+            gene_nlx_compute_host(h, vex, vey, dxg, dyg, pref, rhs, wl.scale)
+            gene_nlx_compute_host(h, vex, vey, dxg, dyg, pref, rhs, 0.0)      # staging buffers are reused; scale 0
+        finally:
+            gene_nlx_destroy(h)
+        assert torch.equal(rhs.to(cuda_device), dev)
+    assert plane_errors(wl, arrs, dev, np.array([0, 1, 9999, planes - 1])).max() <= TOL
+
+
 def test_errors_are_reported(cuda_device):
     from paper_1310_1485_b200 import GeneNLError, gene_nlx_compute, gene_nlx_create, gene_nlx_destroy
     with pytest.raises(GeneNLError):
