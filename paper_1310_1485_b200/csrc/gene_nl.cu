@@ -19,6 +19,7 @@
 #include "../../include/gene_nl_bench.h"
 #include "nl_fused.cuh"
 #include "nl_fused2.cuh"
+#include "nl_cluster.cuh"
 #include "nl_kernels.cuh"
 #include "nl_pipe.cuh"
 
@@ -48,13 +49,35 @@ typedef void (*fused_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cpl
                          double);
 
 typedef void (*fused2_fn)(const cplx*, cplx*, const cplx*, const cplx*, int, int, int, int, double, double, double);
+typedef void (*cluster_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, double, double, double);
 
 struct FusedKernel {
     fused_fn fn = nullptr;
     fused2_fn fn2 = nullptr;  // second-generation kernel (nl_fused2.cuh); used when available
+    cluster_fn fnc = nullptr; // the plane spread over a thread-block cluster (nl_cluster.cuh); chi shared over v only
+    int cluster = 1;          // CTAs per cluster
     size_t smem = 0;
     int nt = 0;
 };
+
+template <int AX, int BX, int AY, int NW>
+FusedKernel make_cluster()
+{
+    using K = gnl::Clustered<AX, BX, AY, NW>;
+    FusedKernel k;
+    k.fnc = gnl::k_plane_cluster<AX, BX, AY, NW>;
+    k.cluster = K::C;
+    k.smem = K::SMEM_BYTES;
+    k.nt = K::NT;
+    return k;
+}
+
+// Planes whose Z exceeds one SM but fits the shared memory of a portable cluster (8 CTAs): 384 x 192 (configs[2])
+bool find_cluster(int nx, int ny, FusedKernel* out)
+{
+    if (nx == 384 && ny == 192) { *out = make_cluster<24, 16, 24, 8>(); return out->smem <= 227 * 1024; }
+    return false;
+}
 
 template <int AX, int AY, int NW>
 FusedKernel make_fused2()
@@ -476,7 +499,21 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const size_t goff = (size_t)s0 * h->nz * h->nv * h->M;
             long long T = (long long)ns * h->nz * h->nv;
             int grid = (T < h->fused_grid) ? (int)T : h->fused_grid;
-            if (h->fk.fn2)
+            if (h->fk.fnc) {
+                // whole clusters only; a cluster walks planes with the stride of the cluster count
+                const int C = h->fk.cluster;
+                long long ncl = (T < h->fused_grid / C) ? T : h->fused_grid / C;
+                cudaLaunchConfig_t cfg = {};
+                cudaLaunchAttribute at[1];
+                cfg.gridDim = dim3((unsigned)(ncl * C));
+                cfg.blockDim = dim3((unsigned)h->fk.nt);
+                cfg.dynamicSmemBytes = h->fk.smem;
+                cfg.stream = st;
+                at[0].id = cudaLaunchAttributeClusterDimension;
+                at[0].val.clusterDim.x = (unsigned)C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+                cfg.attrs = at; cfg.numAttrs = 1;
+                GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fnc, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)h->twx, (const cplx*)h->twy, h->nz, h->nv, ns, h->kxmin, h->kymin, coef)));
+            } else if (h->fk.fn2)
                 GNL_LAUNCH(prof, K_FUSED, (h->fk.fn2<<<grid, h->fk.nt, h->fk.smem, st>>>(g + goff, rhs + goff, s.R, h->twy, h->nz, h->nv, ns, h->chi_has_v, h->kxmin, h->kymin, coef)));
             else
                 GNL_LAUNCH(prof, K_FUSED, (h->fk.fn<<<grid, h->fk.nt, h->fk.smem, st>>>(g + goff, rhs + goff, s.R, h->twx, h->twy, h->nz, h->nv, ns, h->chi_has_v, h->kxmin, h->kymin, coef)));
@@ -553,7 +590,8 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     }
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
     // the composition chi = phi_bar - v_par A_par_bar lives in k_ybracket (batched path)
-    h->fused = !h->em && (find_fused2(h->Nx, h->Ny, &h->fk) || find_fused(h->Nx, h->Ny, &h->fk));
+    h->fused = !h->em && (find_fused2(h->Nx, h->Ny, &h->fk) || find_fused(h->Nx, h->Ny, &h->fk) ||
+                          (!h->chi_has_v && find_cluster(h->Nx, h->Ny, &h->fk)));
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -566,9 +604,24 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
               (!h->em || set_smem(h->yk.br_em, h->yk.smem_br, "k_ybracket(em) smem")) &&
               set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
               set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
-              (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
-                                       : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
+              (!h->fused || (h->fk.fnc ? set_smem(h->fk.fnc, h->fk.smem, "k_plane_cluster smem")
+                             : h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
+                                         : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
               upload_const_twiddles();
+    if (ok && h->fk.fnc) {  // persistent clusters: as many as the device keeps resident at once
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        cfg.gridDim = dim3((unsigned)(h->fk.cluster * (h->fused_grid / h->fk.cluster)));
+        cfg.blockDim = dim3((unsigned)h->fk.nt);
+        cfg.dynamicSmemBytes = h->fk.smem;
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)h->fk.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        int ncl = 0;
+        ok = cuda_ok(cudaOccupancyMaxActiveClusters(&ncl, h->fk.fnc, &cfg), "cudaOccupancyMaxActiveClusters(k_plane_cluster)");
+        if (ok && ncl < 1) { set_err("k_plane_cluster: no cluster fits on the device"); ok = false; }
+        h->fused_grid = ncl * h->fk.cluster;
+    }
     if (ok && h->Nx <= 192) {
         // pipelined persistent x kernel; measured on B200: faster for Nx <= 192 (configs[4]: k_xinv 12.0 -> 10.2 ms),
         // equal at 384, slower at 768
