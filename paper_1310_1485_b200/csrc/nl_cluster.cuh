@@ -53,6 +53,18 @@ __device__ __forceinline__ void st_cluster(uint32_t addr, cplx v)
 {
     asm volatile("st.shared::cluster.v2.f64 [%0], {%1,%2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
 }
+// asynchronous 16-byte store into a peer's shared memory; completes `bytes` on the peer's mbarrier `bar` (both shared::cluster)
+__device__ __forceinline__ void st_async(uint32_t addr, cplx v, uint32_t bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.b64 [%0], {%1,%2}, [%3];" ::"r"(addr),
+                 "l"(__double_as_longlong(v.x)), "l"(__double_as_longlong(v.y)), "r"(bar) : "memory");
+}
+// Arrive on a peer's mbarrier WITHOUT a release fence: used where the arrive only tells the peer that this CTA's
+// loads from a buffer have completed (their values are in registers), so there is nothing to publish.
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t bar_cluster_addr)
+{
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
+}
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
@@ -75,6 +87,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
         "bra GNL_MBAR_WAIT_%=;\n\t"
         "GNL_MBAR_DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
 }
+// wait without an acquire fence (no L1 invalidation): the waiter reads nothing that the arrivals published
+__device__ __forceinline__ void mbar_wait_relaxed(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "GNL_MBARC_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.relaxed.cluster.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra GNL_MBARC_DONE_%=;\n\t"
+        "bra GNL_MBARC_WAIT_%=;\n\t"
+        "GNL_MBARC_DONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
 {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
@@ -96,20 +119,25 @@ struct Clustered {
     // values are in registers by then) and runs FY slots, past the end of the two rows
     static constexpr int PS = (W2 + FY) | 1;
     static constexpr int ZL = PPC * PS;
-    static constexpr int BPX = Tile<AX, BX>::BP, CS = Tile<AX, BX>::STRIDE;
-    static constexpr int E_CPLX = CK * CS;     // x exchange tile of CK columns, one sign at a time
+    // x exchange tile: both signs of the CK columns, HALF of the k1 range at a time (the stage-1 threads keep the other
+    // half in registers), so that every thread has a stage-1 item and E still fits beside Zl
+    static constexpr int BPX = Tile<AX, BX>::BP, AXH = AX / 2, CS = ((AXH * BPX) | 1) + ((((AXH * BPX) | 1) % 8 == 1) ? 4 : 0);
+    static constexpr int E_CPLX = 2 * CK * CS;
     static constexpr int PLS = 2 * CK;         // P_local[pair][slot]: slot = column (+ky), CK + column (-ky)
     static constexpr int PL_CPLX = NPAIR * PLS;
     static constexpr int U_CPLX = E_CPLX > PL_CPLX ? E_CPLX : PL_CPLX;   // E and P_local share one region
     static constexpr int G_CPLX = CK * NX0;    // this CTA's columns of a g plane (one contiguous block)
     static constexpr int TWX = AX * BPX, TWY = AY * 9;
-    static constexpr int SMEM_CPLX = ZL + U_CPLX + G_CPLX + TWX + TWY + 1;   // + one 16-byte slot for the mbarrier
+    static constexpr int NBAR = 3 + NW;        // mbarriers: g block, P_local full, U free, Zl rows of each warp full
+    static constexpr int SMEM_CPLX = ZL + U_CPLX + G_CPLX + TWX + TWY + (NBAR + 2) / 2;   // + the edone counter
+    static constexpr unsigned ZBYTES = NPW * 2 * W2 * 16;   // bytes a warp's pair storages receive per plane
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
     static_assert(AX % 3 == 0 && AY % 3 == 0, "3/2 rule");
     static_assert(BX % 2 == 0 && NKY0 % C == 0 && PPC == AX, "C = BX/2 CTAs: a CTA owns AX row pairs and nky0/C columns");
     static_assert(PPC % NW == 0 && NPW * 8 <= 32 && AY <= 32, "a warp takes NPW pairs: NPW*8 lanes in Y1/Y3, AY lanes in Y2");
     static_assert(CK == 8, "P slots are swizzled over 8-slot halves; 128 B runs in both hand-overs");
-    static_assert(CK * BX <= NT && CK * AX <= NT, "one item per thread in every x stage");
+    static_assert(2 * CK * BX == NT && 2 * CK * AXH <= NT && (2 * CK * AXH) % 32 == 0 && CK * AX <= NT && AX % 2 == 0,
+                  "one item per thread in every x stage; whole warps in stage 2");
     static_assert((G_CPLX * 16) % 16 == 0, "bulk copy size");
 };
 
@@ -133,7 +161,9 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
     cplx* Gs = U + K::U_CPLX;              // this CTA's CK columns of the current g plane (bulk copy)
     cplx* twx = Gs + K::G_CPLX;            // W_NX^{n2 k1}, [k1][BPX]
     cplx* twy = twx + K::TWX;              // W_NY^{k1 k2}, [k1][9]
-    const uint32_t gbar = smem_u32(twy + K::TWY);
+    const uint32_t bars = smem_u32(twy + K::TWY);
+    const uint32_t gbar = bars, pfull = bars + 8, ufree = bars + 16, zfull0 = bars + 24;   // zfull of warp w: zfull0 + 8 w
+    unsigned* edone = (unsigned*)(twy + K::TWY) + 2 * K::NBAR;   // stage-2 warps that have finished with E (this plane)
 
     const int tid = threadIdx.x;
     const int lane0 = tid & 31;
@@ -141,42 +171,61 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
     const uint32_t rank = cluster_ctarank();
     const int ncluster = gridDim.x / C, cl = blockIdx.x / C;
     const uint32_t zl_base = smem_u32(Zl), pl_base = smem_u32(U);
+    const uint32_t pbytes = (uint32_t)(NPAIR * (2 * CK - (rank == 0 ? 1 : 0)) * sizeof(cplx));   // no -ky value for ky = 0
 
     load_twiddles_ab<AX, BX>(twx, twx_g);
     load_twiddles_ab<AY, 8>(twy, twy_g);
     if (tid == 0) {
         mbar_init(gbar, 1);
+        mbar_init(pfull, 1);
+        mbar_init(ufree, C);
+        for (int w = 0; w < NW; ++w) mbar_init(zfull0 + 8 * w, 1);
+        *edone = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    const long long T = (long long)nslab * nz * nv;
+    const unsigned T = (unsigned)nslab * (unsigned)nz * (unsigned)nv;   // planes of this launch (< 2^31: checked by the host)
     const size_t plane_elems = (size_t)NX0 * NKY0;
     // planes are walked v-fastest so that neighbouring clusters share a chi plane in L2
-    auto plane_of = [&](long long tt) {
-        const int v = (int)(tt % nv);
-        const int z = (int)((tt / nv) % nz);
-        const long long sl = tt / ((long long)nv * nz);
+    auto plane_of = [&](unsigned tt) {
+        const unsigned v = tt % (unsigned)nv, zs = tt / (unsigned)nv;
+        const unsigned z = zs % (unsigned)nz, sl = zs / (unsigned)nz;
         return (size_t)z + (size_t)nz * ((size_t)v + (size_t)nv * sl);
     };
-    auto request_g = [&](long long tt) {   // one thread: this CTA's columns of plane tt -> Gs
+    auto request_g = [&](unsigned tt) {   // one thread: this CTA's columns of plane tt -> Gs
         mbar_arrive_expect_tx(gbar, (uint32_t)(K::G_CPLX * sizeof(cplx)));
         bulk_g2s(smem_u32(Gs), g + plane_of(tt) * plane_elems + (size_t)rank * CK * NX0,
                  (uint32_t)(K::G_CPLX * sizeof(cplx)), gbar);
     };
-    if (tid == 0 && cl < T) request_g(cl);
-    // every CTA of the cluster is resident and initialised before anyone stores into it
+    if (tid == 0 && (unsigned)cl < T) request_g((unsigned)cl);
+    // every CTA of the cluster is resident and its mbarriers are initialised before anyone stores into it
     cluster_arrive();
     cluster_wait();
 
-    uint32_t gphase = 0;
-    for (long long t = cl; t < T; t += ncluster) {
+    // shared::cluster address of a peer's copy of a shared::cta address: that address plus a per-peer constant
+    uint32_t peer[C];
+#pragma unroll
+    for (int r = 0; r < C; ++r) peer[r] = mapa_u32(zl_base, (uint32_t)r) - zl_base;
+
+    // Synchronisation inside the plane loop is by mbarriers only (no cluster-wide barrier, so warps whose rows are
+    // complete start while the stores of the others are still in flight):
+    //   zfull[w]  (tx) the 2 W2 NPW values of warp w's pair storages have arrived            -> warp w starts Y
+    //   ufree     (C arrivals) every CTA of the cluster has finished with its exchange tile E -> P may be pushed into U
+    //   pfull     (tx) every P value of this CTA's columns has arrived                        -> X2
+    // A sender is never more than one phase ahead of a receiver: plane p+1's rows are sent after the sender's pfull(p),
+    // which every warp of every CTA completes only after its Y(p); plane p+1's P after zfull(p+1), which needs every
+    // CTA's X1(p+1), which follows its X2(p).  (An mbarrier armed late tolerates one phase of early bytes, not two.)
+    uint32_t ph = 0;
+    for (unsigned t = (unsigned)cl; t < T; t += (unsigned)ncluster, ph ^= 1) {
         const size_t p = plane_of(t);
-        const size_t q = (size_t)((t / nv) % nz) + (size_t)nz * (size_t)(t / ((long long)nv * nz));
+        const size_t q = (size_t)((t / (unsigned)nv) % (unsigned)nz) + (size_t)nz * (size_t)(t / ((unsigned)nv * (unsigned)nz));
         cplx* Rb = rhs + p * plane_elems + (size_t)rank * CK * NX0;
         const cplx* Rc = R + q * ((size_t)NX * NY);
+        if (tid == 0) mbar_arrive_expect_tx(pfull, pbytes);
+        if (lane0 == 0) mbar_arrive_expect_tx(zfull0 + 8 * warp, K::ZBYTES);
         {  // pull the next plane's rhs columns of this CTA towards L2 while this one is being worked on
-            const long long tn = t + ncluster;
+            const unsigned tn = t + (unsigned)ncluster;
             if (tn < T) {
                 const char* b = (const char*)(rhs + plane_of(tn) * plane_elems + (size_t)rank * CK * NX0);
                 for (size_t off = (size_t)tid * 128; off < (size_t)CK * NX0 * sizeof(cplx); off += (size_t)NT * 128)
@@ -185,65 +234,88 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
         }
 
         // =============== X1: derivative, pad, x-synthesis of this CTA's columns; rows go to their owners ===============
-        mbar_wait(gbar, gphase);
-        gphase ^= 1;
-#pragma unroll 1
-        for (int sg = 0; sg < 2; ++sg) {
-            if (tid < CK * BX) {  // stage 1: pruned radix-AX over n1 for fixed n2 (i = n2 + BX n1), twiddle W_NX^{n2 k1}
-                const int n2 = tid % BX, col = tid / BX;
-                const int kyi = (int)rank * CK + col;
-                if (!(sg == 1 && kyi == 0)) {  // there is no -0 column
-                    const cplx* Fc = Gs + col * NX0;
-                    const double ky = kymin * (double)kyi;
-                    const double kys = sg ? ky : -ky;  // (i kx - ky) F for +ky, (i kx + ky) F for -ky
-                    cplx lo[AX1], hi[AX1];
-#pragma unroll
-                    for (int a = 0; a < AX1; ++a) {
-                        const int i0 = n2 + BX * a, i1 = i0 + M;
-                        cplx f0 = Fc[i0], f1 = Fc[i1];
-                        if (kyi == 0) {  // Hermitian part of the ky = 0 column (reading R7)
-                            const cplx m0 = Fc[(NX0 - i0) % NX0], m1 = Fc[NX0 - i1];
-                            f0 = cmake(0.5 * (f0.x + m0.x), 0.5 * (f0.y - m0.y));
-                            f1 = cmake(0.5 * (f1.x + m1.x), 0.5 * (f1.y - m1.y));
-                        }
-                        lo[a] = deriv_mul(f0, kxmin * (double)i0, kys);
-                        hi[a] = (i1 == M) ? cmake(0.0, 0.0) : deriv_mul(f1, kxmin * (double)(i1 - NX0), kys);  // Nyquist row (R6)
-                    }
-                    cplx out[AX];
-                    dft_pruned_in<AX, +1>(lo, hi, out);
-                    cplx* Ec = U + col * CS + n2;
-#pragma unroll
-                    for (int k1 = 0; k1 < AX; ++k1) {
-                        const cplx w = twx[k1 * BPX + n2];
-                        Ec[k1 * BPX] = (k1 == 0) ? out[0] : cmul(out[k1], w.x, w.y);
-                    }
-                }
+        mbar_wait(gbar, ph);
+        if (rank == 0) {   // Hermitian part of the ky = 0 column (reading R7), in place in the staged block
+            if (tid > 0 && tid < NX0 / 2) {
+                const cplx a = Gs[tid], b = Gs[NX0 - tid];
+                Gs[tid] = cmake(0.5 * (a.x + b.x), 0.5 * (a.y - b.y));
+                Gs[NX0 - tid] = cmake(0.5 * (a.x + b.x), 0.5 * (b.y - a.y));
+            } else if (tid == 0) {
+                Gs[0].y = 0.0;
             }
             __syncthreads();
-            // the g block is consumed after the second sign's stage 1: ask for the next plane's
-            if (sg == 1 && tid == 0 && t + ncluster < T) request_g(t + ncluster);
-            if (tid < CK * AX) {  // stage 2: radix-BX over n2 for fixed k1; row m = k1 + AX k2 -> CTA k2 mod C, pair k1
-                const int col = tid % CK, k1 = tid / CK;
-                const int kyi = (int)rank * CK + col;
-                const bool zero = (sg == 1 && kyi == 0);
-                cplx v[BX];
-                const cplx* Ec = U + col * CS + k1 * BPX;
+        }
+        {
+            // stage 1, every thread: column-sign c2 = (sign, column), position n2: pruned radix-AX over n1 (i = n2 + BX n1),
+            // twiddle W_NX^{n2 k1}.  The k1 < AX/2 half goes to E now, the other half after the first stage-2 pass.
+            const int n2 = opaque(tid % BX), c2 = opaque(tid / BX);
+            cplx out[AX];
+            {
+                const int col1 = c2 % CK;
+                const cplx* Fc = Gs + col1 * NX0 + n2;
+                const double ky = kymin * (double)((int)rank * CK + col1), dn2 = (double)n2;
+                const double kys = (c2 / CK) ? ky : -ky;  // (i kx - ky) F for +ky, (i kx + ky) F for -ky
+                cplx lo[AX1], hi[AX1];
 #pragma unroll
-                for (int n2 = 0; n2 < BX; ++n2) v[n2] = zero ? cmake(0.0, 0.0) : Ec[n2];
-                Dft<BX, +1>::run(v);
-                const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
-                const uint32_t a0 = zl_base + (uint32_t)((k1 * PS + cc) * sizeof(cplx));
+                for (int a = 0; a < AX1; ++a) {
+                    lo[a] = deriv_mul(Fc[BX * a], kxmin * (dn2 + (double)(BX * a)), kys);                // i = n2 + BX a      (kx >= 0)
+                    hi[a] = deriv_mul(Fc[BX * a + M], kxmin * (dn2 + (double)(BX * a + M - NX0)), kys);  // i = n2 + BX a + M  (kx < 0)
+                }
+                if (n2 == 0) hi[0] = cmake(0.0, 0.0);  // i = M: the Nyquist row is ignored (R6)
+                dft_pruned_in<AX, +1>(lo, hi, out);
 #pragma unroll
-                for (int k2 = 0; k2 < BX; ++k2) {
-                    // half 0 (row m < NX/2) sits at [W2, 2 W2), half 1 at [0, W2)
-                    const uint32_t a = mapa_u32(a0 + (uint32_t)((k2 < C ? W2 : 0) * sizeof(cplx)), (uint32_t)(k2 % C));
-                    st_cluster(a, sg ? cconj(v[k2]) : v[k2]);
+                for (int k1 = 1; k1 < AX; ++k1) {
+                    const cplx w = twx[k1 * BPX + n2];
+                    out[k1] = cmul(out[k1], w.x, w.y);
                 }
             }
-            __syncthreads();  // E is free for the next sign / for the incoming P
+            __syncthreads();   // every thread has read its g values
+            if (tid == 0 && t + (unsigned)ncluster < T) request_g(t + (unsigned)ncluster);   // the next plane's block, a plane ahead
+#pragma unroll
+            for (int hk = 0; hk < 2; ++hk) {
+                {
+                    cplx* Ec = U + c2 * CS + n2;
+#pragma unroll
+                    for (int k1 = 0; k1 < K::AXH; ++k1) Ec[k1 * BPX] = out[hk * K::AXH + k1];
+                }
+                __syncthreads();
+                if (tid < 2 * CK * K::AXH) {
+                    // stage 2: radix-BX over n2 for fixed k1; row m = k1 + AX k2 -> CTA k2 mod C, pair storage k1.
+                    // Lanes run over the 2 CK column-signs: two 128 B runs per store instruction and k1 value.
+                    const int c2s = tid % (2 * CK), k1 = hk * K::AXH + tid / (2 * CK);
+                    const int sg = c2s / CK, kyi = (int)rank * CK + c2s % CK;
+                    const bool zero = (sg == 1 && kyi == 0);  // there is no -0 column: slot cc = nky0 holds zeros
+                    cplx v[BX];
+                    const cplx* Ec = U + c2s * CS + (k1 - hk * K::AXH) * BPX;
+#pragma unroll
+                    for (int i = 0; i < BX; ++i) v[i] = zero ? cmake(0.0, 0.0) : Ec[i];
+                    Dft<BX, +1>::run(v);
+                    const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
+                    const uint32_t a0 = zl_base + (uint32_t)((k1 * PS + cc) * sizeof(cplx));
+                    const uint32_t zb = zfull0 + 8 * (uint32_t)(k1 / NPW);   // the warp that owns pair k1 at the receiver
+                    const double sgn = sg ? -1.0 : 1.0;                      // -ky columns hold the conjugate
+#pragma unroll
+                    for (int k2 = 0; k2 < BX; ++k2) {
+                        // half 0 (row m < NX/2) sits at [W2, 2 W2), half 1 at [0, W2)
+                        st_async(a0 + (uint32_t)((k2 < C ? W2 : 0) * sizeof(cplx)) + peer[k2 % C],
+                                 cmake(v[k2].x, sgn * v[k2].y), zb + peer[k2 % C]);
+                    }
+                    if (hk == 1) {
+                        // The last stage-2 warp to get here tells every CTA of the cluster that this CTA's U may
+                        // receive P from now on (all loads from E have completed: their values went into the stores).
+                        // No CTA barrier: the warps without a stage-2 item are already waiting for their rows.
+                        __syncwarp(FULL);
+                        if (lane0 == 0 && atomicAdd(edone, 1u) == (unsigned)(2 * CK * K::AXH / 32 - 1)) {
+                            *edone = 0;
+#pragma unroll
+                            for (int r = 0; r < C; ++r) mbar_arrive_remote_relaxed(ufree + peer[r]);
+                        }
+                    }
+                }
+                if (hk == 0) __syncthreads();  // E is free for the second half
+            }
         }
-        cluster_arrive();
-        // chi rows of this warp's first pair, requested while the cluster gathers
+        // chi rows of this warp's first pair, requested while the rows arrive
         const int lane = opaque(lane0);
         const int k1y = lane < AY ? lane : lane - AY;   // lanes >= AY shadow an item (same addresses) and skip the stores
         const bool act2 = lane < AY;
@@ -254,7 +326,7 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
 #pragma unroll
             for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
         }
-        cluster_wait();
+        mbar_wait(zfull0 + 8 * warp, ph);
 
         // =============== Y: this warp's NPW row pairs, __syncwarp only ===============
         {
@@ -288,6 +360,16 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
                 __syncwarp(FULL);
 #pragma unroll
                 for (int j = 0; j < NPW; ++j) {  // Y2: twiddle + radix-8 to real space, bracket; pair j, k1 = lane
+                    // chi rows of the NEXT item (pair j+1 of this half, or pair 0 of the second half), requested before
+                    // this item's butterflies so that their latency hides behind them
+                    cplx chn[8];
+                    const int jn = (j + 1 < NPW) ? j + 1 : 0, hn = (j + 1 < NPW) ? h : 1;
+                    if (!(h == 1 && j + 1 == NPW)) {
+                        const int m = (int)rank * PPC + warp * NPW + jn + hn * NPAIR;
+                        const cplx* Rr = Rc + (size_t)m * NY + k1y;
+#pragma unroll
+                        for (int k2 = 0; k2 < 8; ++k2) chn[k2] = ldg_nc_early(Rr + AY * k2);
+                    }
                     cplx* tile = Zw + j * PS + W2 + k1y * 9;
                     cplx v[8];
 #pragma unroll
@@ -309,13 +391,9 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
                             for (int k2 = 0; k2 < 8; ++k2) tile[k2] = w[k2];
                         }
                     }
-                    // chi rows of the next item: pair j+1 of this half, or pair 0 of the second half
-                    const int jn = (j + 1 < NPW) ? j + 1 : 0, hn = (j + 1 < NPW) ? h : 1;
                     if (!(h == 1 && j + 1 == NPW)) {
-                        const int m = (int)rank * PPC + warp * NPW + jn + hn * NPAIR;
-                        const cplx* Rr = Rc + (size_t)m * NY + k1y;
 #pragma unroll
-                        for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
+                        for (int k2 = 0; k2 < 8; ++k2) chv[k2] = chn[k2];
                     }
                 }
                 __syncwarp(FULL);
@@ -327,6 +405,7 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
                 for (int n1 = 0; n1 < AY; ++n1) in[n1] = tile[n1 * 9];
                 cplx lo[AY1], hi[AY1];
                 dft_pruned_out<AY, -1>(in, lo, hi);
+                mbar_wait_relaxed(ufree, ph);   // every CTA of the cluster is done with its exchange tile
                 if (act1) {
                     const int qg = (int)rank * PPC + warp * NPW + j1;   // global pair index = row of P_local
                     const uint32_t row = pl_base + (uint32_t)(qg * PLS * sizeof(cplx));
@@ -335,19 +414,19 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
                     for (int c = 0; c < AY1; ++c) {
                         {  // +ky half: ky = n2 + 8 c
                             const int ky = n2 + 8 * c;
-                            st_cluster(mapa_u32(row + (uint32_t)(((ky % CK) ^ sw) * sizeof(cplx)), (uint32_t)(ky / CK)), lo[c]);
+                            st_async(row + (uint32_t)(((ky % CK) ^ sw) * sizeof(cplx)) + peer[c], lo[c], pfull + peer[c]);
                         }
                         {  // -ky half: cc = nky0 + n2 + 8 c  <->  ky = nky0 - n2 - 8 c (ky = nky0 is a deleted mode)
                             const int ky = NKY0 - n2 - 8 * c;
+                            const uint32_t dl = n2 ? peer[C - 1 - c] : peer[(C - c) % C];   // owner ky / CK
                             if (ky < NKY0)
-                                st_cluster(mapa_u32(row + (uint32_t)((CK + ((ky % CK) ^ sw)) * sizeof(cplx)), (uint32_t)(ky / CK)), hi[c]);
+                                st_async(row + (uint32_t)((CK + ((ky % CK) ^ sw)) * sizeof(cplx)) + dl, hi[c], pfull + dl);
                         }
                     }
                 }
             }
         }
-        cluster_arrive();
-        // rhs values of this thread's share of X2 stage 2, requested while the cluster gathers
+        // rhs values of this thread's share of X2 stage 2, requested while the P rows arrive
         cplx r0[AX1], r1[AX1];
         const int k2s = tid % BX, cols = (tid / BX) % CK;
         if (tid < CK * BX) {
@@ -358,7 +437,7 @@ k_plane_cluster(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* 
                 r1[c] = ldg_early(Rcol + BX * c + M);
             }
         }
-        cluster_wait();
+        mbar_wait(pfull, ph);
 
         // =============== X2: x-analysis of this CTA's columns in place over P_local; delete modes, prefactor, add ===============
         cplx* Pl = U;
