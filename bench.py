@@ -442,7 +442,7 @@ def measured_traffic(workload_name):
     return rows, None
 
 
-def run_config(wl, args, env, do_e2e, do_cpu, headline):
+def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
     """Time one workload: device-resident steps (CUDA events on the launching stream, max over ranks), per-kernel
     rooflines (event pair per launch), e2e through the host entry point, the oracle as cpu_baseline."""
     import torch
@@ -470,7 +470,7 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline):
         my = W.Workload(wl.name, wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin,
                         wl.chi_has_v, wl.seed + 1000 * rank, wl.rhs_random, wl.scale)
     chi, g, rhs = W.make_inputs(my, dev)
-    nl = GeneNL(my)
+    nl = GeneNL(my, plane_kernel=plane_kernel)
     stream = torch.cuda.current_stream()
     warm = max(args.warmup, 3)
     w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -534,7 +534,7 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline):
                           "tflops": flops[k] * nprof / (prof_ms[k] * 1e-3) / 1e12}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
     # measured DRAM bytes (ncu capture of these very sources; null when the capture is older than the code)
-    cap, why = measured_traffic(wl.name)
+    cap, why = measured_traffic(wl.name + ("+cluster" if plane_kernel else ""))
     traffic = cap[dom][0] if dom in cap else None
     traffic_step = None
     if cap and all(k in cap for k in kernels):
@@ -633,6 +633,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="headline configuration only")
+    ap.add_argument("--cluster", action="store_true", help="select the cluster kernel (configs[2]-sized planes only)")
     ap.add_argument("--xglobal", action="store_true",
                     help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
     ap.add_argument("--strong", action="store_true",
@@ -677,7 +678,10 @@ def main():
         pass
     env = {"dev": dev, "dist": dist, "world": world, "rank": rank, "local_rank": local_rank, "peaks": peaks}
 
-    res = run_config(wl, args, env, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, headline=True)
+    pk = None
+    if args.cluster:
+        from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER as pk
+    res = run_config(wl, args, env, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, headline=True, plane_kernel=pk)
     per_config = None
     if args.config is None and world == 1 and not args.no_per_config:
         # the other target configurations, device-resident, in the same run (same box, same clocks record)
@@ -687,6 +691,11 @@ def main():
             per_config[W.CONFIGS[idx].name] = {k: r[k] for k in ("value", "ms_per_step", "steps", "roofline",
                                                                   "roofline_step", "kernels", "clocks", "gpu_launches")}
             per_config[W.CONFIGS[idx].name]["unit"] = UNIT
+        # configs[2] once more through the cluster kernel (Z and P in distributed shared memory instead of HBM scratch)
+        from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER
+        r = run_config(W.CONFIGS[2], args, env, do_e2e=False, do_cpu=False, headline=False, plane_kernel=GENE_NL_KERNEL_CLUSTER)
+        per_config[W.CONFIGS[2].name + " (gene_nl_set_plane_kernel: cluster kernel)"] = {
+            k: r[k] for k in ("value", "ms_per_step", "steps", "roofline", "roofline_step", "kernels", "clocks", "gpu_launches")}
     if rank == 0:
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": res["steps"],

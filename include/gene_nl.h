@@ -127,11 +127,28 @@ int gene_nl_set_scratch_bytes(gene_nl_plan* h, size_t bytes);
 int gene_nl_launches_per_compute(const gene_nl_plan* h);
 
 /*
+ * gene_nl_set_plane_kernel -- choose the kernel family for the g side of a plane.
+ *   GENE_NL_KERNEL_AUTO     what gene_nl_create selected (the fastest measured on B200): the fused shared-memory kernel
+ *                           for planes that fit one SM, the batched kernels (scratch through HBM/L2) beyond.
+ *   GENE_NL_KERNEL_CLUSTER  the fused kernel spread over a thread-block cluster of 8 CTAs: the half-transformed plane is
+ *                           distributed over the cluster's shared memory and the two x<->y hand-overs (the
+ *                           "transpositions" of PAPER.md:61) are distributed-shared-memory stores, so only g, rhs and
+ *                           the chi rows cross HBM (1.03 x the algorithmic bytes).  Available for the 384 x 192 padded
+ *                           grid (nx0 = 256, nky0 = 64: configs[2]) with chi_has_v = 0; GENE_NL_EUNSUPPORTED otherwise.
+ * Same results to rounding (both are checked against the oracle).  Synchronises the device and re-allocates the
+ * scratch, like gene_nl_set_scratch_bytes.
+ */
+#define GENE_NL_KERNEL_AUTO 0
+#define GENE_NL_KERNEL_CLUSTER 1
+int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind);
+
+/*
  * gene_nl_query -- plan facts for benchmarks and tests.  `what`:
  *   0 planes, 1 Nx, 2 Ny, 3 planes per batch, 4 batches per compute,
  *   5 algorithmic bytes per plane  B = 16*nx0*nky0*(3 + c),
  *   6 conventional flops per plane F = (3+2c)*T2D + 4M(1+c) + 3NxNy + 4M,
- *   with c = 1 if chi_has_v else 1/nv; 7: 1 if the fused shared-memory kernel is used, else 0.
+ *   with c = 1 if chi_has_v else 1/nv; 7: 1 if a fused (shared-memory resident) kernel is used, else 0;
+ *   8: 1 if that kernel is the cluster kernel (gene_nl_set_plane_kernel), else 0.
  *   Returns NaN for an unknown `what` or NULL plan.
  */
 double gene_nl_query(const gene_nl_plan* h, int what);

@@ -18,7 +18,7 @@ GENE_NL_OK, GENE_NL_EINVAL, GENE_NL_EUNSUPPORTED, GENE_NL_ECUDA, GENE_NL_ENOMEM 
 # every symbol include/gene_nl.h declares (the product boundary) ...
 EXPORTED_SYMBOLS = (
     "gene_nl_create", "gene_nl_compute", "gene_nl_compute_em", "gene_nl_compute_host", "gene_nl_compute_em_host",
-    "gene_nl_destroy", "gene_nl_last_error", "gene_nl_set_scratch_bytes",
+    "gene_nl_destroy", "gene_nl_last_error", "gene_nl_set_scratch_bytes", "gene_nl_set_plane_kernel",
     "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query",
     "gene_nlx_create", "gene_nlx_compute", "gene_nlx_compute_host", "gene_nlx_destroy", "gene_nlx_query",
 )
@@ -62,6 +62,8 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_compute_em_host.restype = i
         lib.gene_nl_set_scratch_bytes.argtypes = [vp, ctypes.c_size_t]
         lib.gene_nl_set_scratch_bytes.restype = i
+        lib.gene_nl_set_plane_kernel.argtypes = [vp, i]
+        lib.gene_nl_set_plane_kernel.restype = i
         lib.gene_nl_destroy.argtypes = [vp]
         lib.gene_nl_destroy.restype = None
         lib.gene_nl_last_error.argtypes = []
@@ -153,6 +155,16 @@ def gene_nl_set_scratch_bytes(h, nbytes: int) -> None:
     rc = load_library().gene_nl_set_scratch_bytes(h, int(nbytes))
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_set_scratch_bytes failed ({rc}): {gene_nl_last_error()}")
+
+
+GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER = 0, 1
+
+
+def gene_nl_set_plane_kernel(h, kind: int) -> None:
+    """Kernel family for the g side of a plane: GENE_NL_KERNEL_AUTO or GENE_NL_KERNEL_CLUSTER (see include/gene_nl.h)."""
+    rc = load_library().gene_nl_set_plane_kernel(h, int(kind))
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_set_plane_kernel failed ({rc}): {gene_nl_last_error()}")
 
 
 KERNEL_CLASSES = ("k_xinv", "k_yreal", "k_ybracket", "k_xfwd", "k_plane_fused")
@@ -248,9 +260,11 @@ def gene_nlx_query(h, what: int) -> float:
 class GeneNL:
     """Context-manager convenience around create/compute/destroy for a workloads.Workload."""
 
-    def __init__(self, wl, scratch_bytes=None):
+    def __init__(self, wl, scratch_bytes=None, plane_kernel=None):
         self.wl = wl
         self.h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, wl.chi_has_v)
+        if plane_kernel is not None:
+            gene_nl_set_plane_kernel(self.h, plane_kernel)
         if scratch_bytes is not None:
             gene_nl_set_scratch_bytes(self.h, scratch_bytes)
 

@@ -281,6 +281,11 @@ struct gene_nl_plan {
     XKernels xk;
     YKernels yk;
     FusedKernel fk;
+    FusedKernel ck;           // the cluster kernel for this plane size, if there is one (gene_nl_set_plane_kernel)
+    int ck_grid = 0;          // its grid: resident clusters x CTAs per cluster
+    FusedKernel fk_auto;      // what gene_nl_create selected
+    bool fused_auto = false;
+    int fused_grid_auto = 0;
     bool fused = false;
     int fused_grid = 0;
     int nss = 1;      // fused: (w,s) slabs per launch (Rchi of that many slabs is kept)
@@ -358,6 +363,7 @@ void configure_batching(gene_nl_plan* h)
         size_t nss = rcap / (cps * rpp);
         if (nss < 1) nss = 1;
         if (nss > (size_t)h->nw * h->nspec) nss = (size_t)h->nw * h->nspec;
+        while (nss > 1 && nss * (size_t)nz * nv >= ((size_t)1 << 31)) nss /= 2;   // 32-bit plane counters in the kernels
         h->nss = (int)nss;
         const size_t zcap = (h->budget_set && budget < ((size_t)64 << 20)) ? budget : (size_t)64 << 20;
         size_t nbz = zcap / zpp;
@@ -590,8 +596,12 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     }
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
     // the composition chi = phi_bar - v_par A_par_bar lives in k_ybracket (batched path)
-    h->fused = !h->em && (find_fused2(h->Nx, h->Ny, &h->fk) || find_fused(h->Nx, h->Ny, &h->fk) ||
-                          (!h->chi_has_v && find_cluster(h->Nx, h->Ny, &h->fk)));
+    h->fused = !h->em && (find_fused2(h->Nx, h->Ny, &h->fk) || find_fused(h->Nx, h->Ny, &h->fk));
+    // Planes beyond one SM: the batched kernels by default.  The cluster kernel (nl_cluster.cuh) keeps Z and P out of
+    // HBM (1.03 x the algorithmic bytes, ncu) but measured slower on B200 (configs[2]: 8.2 ms against 7.2 ms: only 15
+    // clusters of 8 CTAs are co-resident on the 148 SMs, and the DSMEM hand-overs run at 18 B/clk/SM in series with the
+    // butterflies; DESIGN.md sect. 6e), so it is selected on request only (gene_nl_set_plane_kernel).
+    if (!h->fused && !h->em && !h->chi_has_v) find_cluster(h->Nx, h->Ny, &h->ck);
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -604,24 +614,30 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
               (!h->em || set_smem(h->yk.br_em, h->yk.smem_br, "k_ybracket(em) smem")) &&
               set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
               set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
-              (!h->fused || (h->fk.fnc ? set_smem(h->fk.fnc, h->fk.smem, "k_plane_cluster smem")
-                             : h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
-                                         : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
+              (!h->ck.fnc || set_smem(h->ck.fnc, h->ck.smem, "k_plane_cluster smem")) &&
+              (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
+                                       : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
               upload_const_twiddles();
-    if (ok && h->fk.fnc) {  // persistent clusters: as many as the device keeps resident at once
+    if (ok && h->ck.fnc) {  // persistent clusters: as many as the device keeps resident at once
+        int sms = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
-        cfg.gridDim = dim3((unsigned)(h->fk.cluster * (h->fused_grid / h->fk.cluster)));
-        cfg.blockDim = dim3((unsigned)h->fk.nt);
-        cfg.dynamicSmemBytes = h->fk.smem;
+        cfg.gridDim = dim3((unsigned)(h->ck.cluster * ((sms > 0 ? sms : 148) / h->ck.cluster)));
+        cfg.blockDim = dim3((unsigned)h->ck.nt);
+        cfg.dynamicSmemBytes = h->ck.smem;
         at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = (unsigned)h->fk.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        at[0].val.clusterDim.x = (unsigned)h->ck.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         int ncl = 0;
-        ok = cuda_ok(cudaOccupancyMaxActiveClusters(&ncl, h->fk.fnc, &cfg), "cudaOccupancyMaxActiveClusters(k_plane_cluster)");
-        if (ok && ncl < 1) { set_err("k_plane_cluster: no cluster fits on the device"); ok = false; }
-        h->fused_grid = ncl * h->fk.cluster;
+        if (cudaOccupancyMaxActiveClusters(&ncl, h->ck.fnc, &cfg) != cudaSuccess || ncl < 1) {
+            cudaGetLastError();
+            h->ck = FusedKernel();   // no cluster of that size fits this device: the option is not offered
+        } else {
+            h->ck_grid = ncl * h->ck.cluster;
+        }
     }
+    h->fk_auto = h->fk; h->fused_auto = h->fused; h->fused_grid_auto = h->fused_grid;
     if (ok && h->Nx <= 192) {
         // pipelined persistent x kernel; measured on B200: faster for Nx <= 192 (configs[4]: k_xinv 12.0 -> 10.2 ms),
         // equal at 384, slower at 768
@@ -718,6 +734,26 @@ int gene_nl_set_scratch_bytes(gene_nl_plan* h, size_t bytes)
         g_err = keep;
         return GENE_NL_ENOMEM;
     }
+    return GENE_NL_OK;
+}
+
+int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
+{
+    g_err.clear();
+    if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
+    if (kind != GENE_NL_KERNEL_AUTO && kind != GENE_NL_KERNEL_CLUSTER) { set_err("gene_nl_set_plane_kernel: unknown kind"); return GENE_NL_EINVAL; }
+    if (kind == GENE_NL_KERNEL_CLUSTER && !h->ck.fnc) {
+        set_err("gene_nl_set_plane_kernel: no cluster kernel for this plan (384 x 192 padded grid, chi shared over v, a device that keeps clusters of 8 CTAs resident)");
+        return GENE_NL_EUNSUPPORTED;
+    }
+    if (!on_plan_device(h)) return GENE_NL_EINVAL;
+    if (!cuda_ok(cudaDeviceSynchronize(), "cudaDeviceSynchronize")) return GENE_NL_ECUDA;
+    free_stages(h);
+    free_scratch(&h->scr);
+    if (kind == GENE_NL_KERNEL_CLUSTER) { h->fk = h->ck; h->fused = true; h->fused_grid = h->ck_grid; }
+    else { h->fk = h->fk_auto; h->fused = h->fused_auto; h->fused_grid = h->fused_grid_auto; }
+    configure_batching(h);
+    if (!alloc_scratch(h, &h->scr)) { free_scratch(&h->scr); return GENE_NL_ENOMEM; }
     return GENE_NL_OK;
 }
 
@@ -939,6 +975,7 @@ double gene_nl_query(const gene_nl_plan* h, int what)
     case 4: return h->fused ? (double)((h->nw * h->nspec + h->nss - 1) / h->nss)
                             : (double)h->nw * h->nspec * chunks_per_slab(h) * ((h->nv + h->nvb - 1) / h->nvb);
     case 7: return h->fused ? 1.0 : 0.0;
+    case 8: return h->fk.fnc ? 1.0 : 0.0;
     case 5: return 16.0 * M * (3.0 + c);
     case 6: {
         const double t2d = h->nky0 * 5.0 * Nx * std::log2(Nx) + Nx * 2.5 * Ny * std::log2(Ny);

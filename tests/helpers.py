@@ -61,11 +61,11 @@ def plane_max_errors(wl, out_planes, ref, R_in):
     return num / den
 
 
-def gpu_compute(wl, chi, g, rhs, scale=None, host=False, scratch_bytes=None):
+def gpu_compute(wl, chi, g, rhs, scale=None, host=False, scratch_bytes=None, plane_kernel=None):
     """rhs += scale*N through the C ABI; returns the updated rhs tensor (a new tensor)."""
     from paper_1310_1485_b200 import GeneNL
     out = rhs.clone()
-    with GeneNL(wl, scratch_bytes=scratch_bytes) as nl:
+    with GeneNL(wl, scratch_bytes=scratch_bytes, plane_kernel=plane_kernel) as nl:
         if host:
             nl.compute_host(chi, g, out, scale)
         else:
@@ -74,11 +74,12 @@ def gpu_compute(wl, chi, g, rhs, scale=None, host=False, scratch_bytes=None):
     return out
 
 
-def check_parity(wl, device, nsample=None, host=False, tol=TOL, backend=oracle.DFT_RECURSIVE, scratch_bytes=None):
+def check_parity(wl, device, nsample=None, host=False, tol=TOL, backend=oracle.DFT_RECURSIVE, scratch_bytes=None,
+                 plane_kernel=None):
     chi, g, rhs = W.make_inputs(wl, device if not host else "cpu")
     if host:
         chi, g, rhs = chi.pin_memory(), g.pin_memory(), rhs.pin_memory()
-    out = gpu_compute(wl, chi, g, rhs, host=host, scratch_bytes=scratch_bytes)
+    out = gpu_compute(wl, chi, g, rhs, host=host, scratch_bytes=scratch_bytes, plane_kernel=plane_kernel)
     planes = np.arange(wl.planes) if nsample is None or nsample >= wl.planes else sample_planes(wl, nsample, wl.seed)
     err, emax = [], []
     for c0 in range(0, len(planes), 1024):   # the oracle in bounded chunks (host memory)

@@ -148,13 +148,13 @@ def test_errors_are_reported_not_swallowed(cuda_device):
         torch.cuda.synchronize()
 
 
-def _full_size(cuda_device, idx, nsample):
+def _full_size(cuda_device, idx, nsample, plane_kernel=None):
     wl = W.CONFIGS[idx]
     need = 16 * wl.nx0 * wl.nky0 * (3 * wl.planes + wl.chi_planes) * 1.15
     free, _ = torch.cuda.mem_get_info()
     if free < need:
         pytest.skip(f"{wl.name} needs {need / 2**30:.0f} GiB of device memory")
-    return check_parity(wl, cuda_device, nsample=nsample)
+    return check_parity(wl, cuda_device, nsample=nsample, plane_kernel=plane_kernel)
 
 
 def test_config1_full_size_all_planes(cuda_device):
@@ -190,6 +190,62 @@ def test_plane_sharded_ranks_assemble_to_the_unsharded_result(cuda_device, world
         assert torch.equal(torch.cat(parts), whole.reshape(-1))
 
 
+# ---- the cluster kernel (gene_nl_set_plane_kernel(GENE_NL_KERNEL_CLUSTER)): 384 x 192 planes over 8 CTAs, DSMEM hand-overs ----
+CLUSTER_SHAPES = [(256, 64, 1, 1, 1, 1),       # one plane: one cluster busy, the others idle
+                  (256, 64, 2, 3, 1, 1),
+                  (256, 64, 3, 5, 2, 2),       # 60 planes: several planes per cluster, chi shared by 5 planes
+                  (256, 64, 36, 2, 1, 1)]
+
+
+@pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec", CLUSTER_SHAPES)
+def test_cluster_kernel_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, nw, nspec):
+    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER, GeneNL
+    wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, False, seed=300 + nz + nv)
+    with GeneNL(wl, plane_kernel=GENE_NL_KERNEL_CLUSTER) as nl:
+        assert nl.query(7) == 1.0 and nl.query(8) == 1.0         # the cluster kernel is the one that runs
+    check_parity(wl, cuda_device, plane_kernel=GENE_NL_KERNEL_CLUSTER)
+    check_parity(wl, cuda_device, plane_kernel=GENE_NL_KERNEL_CLUSTER, scratch_bytes=20 << 20)   # several launches
+    check_parity(wl, cuda_device, plane_kernel=GENE_NL_KERNEL_CLUSTER, host=True)                 # behind the streaming driver
+
+
+def test_cluster_kernel_config2_full_size_all_planes(cuda_device):
+    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER
+    _full_size(cuda_device, 2, None, plane_kernel=GENE_NL_KERNEL_CLUSTER)
+
+
+def test_cluster_kernel_properties_and_selection(cuda_device):
+    from paper_1310_1485_b200 import (GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER, GeneNL, GeneNLError,
+                                      gene_nl_set_plane_kernel)
+    wl = W.small_workload(256, 64, 2, 3, 1, 2, 0.05, 0.05, False, seed=61)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    kw = dict(plane_kernel=GENE_NL_KERNEL_CLUSTER)
+    assert torch.equal(gpu_compute(wl, chi, g, rhs, scale=0.0, **kw), rhs)          # scale = 0: bit-identical
+    a = gpu_compute(wl, chi, g, rhs, **kw)
+    assert torch.equal(a, gpu_compute(wl, chi, g, rhs, **kw))                       # deterministic
+    b = gpu_compute(wl, chi, g, rhs)                                                # the batched kernels (default)
+    assert (a - b).abs().max() <= 1e-13 * (b - rhs).abs().max()
+    h = wl.nx0 // 2
+    assert torch.equal(W.as_planes(a, wl)[:, :, h], W.as_planes(rhs, wl)[:, :, h])  # Nyquist row untouched
+    with GeneNL(wl) as nl:                                                          # switching back and forth on one plan
+        assert nl.query(8) == 0.0
+        gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_CLUSTER)
+        out = rhs.clone()
+        nl.compute(chi, g, out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, a)
+        gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_AUTO)
+        out = rhs.clone()
+        nl.compute(chi, g, out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, b)
+        with pytest.raises(GeneNLError):
+            gene_nl_set_plane_kernel(nl.h, 7)
+    for bad in (W.small_workload(128, 32, 1, 1, 1, 1), W.small_workload(256, 64, 1, 1, 1, 1, chi_has_v=True)):
+        with GeneNL(bad) as nl:
+            with pytest.raises(GeneNLError):
+                gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_CLUSTER)                  # no cluster kernel for these
+
+
 def test_config1_sampled_modes_against_the_definition(cuda_device):
     """Sampled outputs the definition can compute one by one, at BASELINE.json's full size."""
     wl = W.CONFIGS[1]
@@ -209,12 +265,14 @@ def test_compute_is_capturable_in_a_cuda_graph(cuda_device):
     """gene_nl_compute only enqueues kernels on the caller's stream (no synchronisation, no allocation): it can be
     captured into a CUDA graph and replayed; fused and batched paths."""
     from paper_1310_1485_b200 import GeneNL
-    for wl in (W.small_workload(128, 32, 2, 3, 1, 1, 0.05, 0.05, False, seed=41),     # fused kernel
-               W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, True, seed=42)):     # batched kernels
+    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER
+    for wl, pk in ((W.small_workload(128, 32, 2, 3, 1, 1, 0.05, 0.05, False, seed=41), None),     # fused kernel
+                   (W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, True, seed=42), None),      # batched kernels
+                   (W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, False, seed=43), GENE_NL_KERNEL_CLUSTER)):
         chi, g, rhs = W.make_inputs(wl, cuda_device)
-        expect = gpu_compute(wl, chi, g, rhs)
+        expect = gpu_compute(wl, chi, g, rhs, plane_kernel=pk)
         out = rhs.clone()
-        with GeneNL(wl) as nl:
+        with GeneNL(wl, plane_kernel=pk) as nl:
             side = torch.cuda.Stream()
             side.wait_stream(torch.cuda.current_stream())
             with torch.cuda.stream(side):
