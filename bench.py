@@ -634,6 +634,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-per-config", action="store_true", help="headline configuration only")
     ap.add_argument("--cluster", action="store_true", help="select the cluster kernel (configs[2]-sized planes only)")
+    ap.add_argument("--plane-kernel", type=int, default=None, help="gene_nl_set_plane_kernel kind (1 cluster, 2 group, 3 batched)")
     ap.add_argument("--xglobal", action="store_true",
                     help="x-global variant (SURVEY 8(f) f2): the paper's 64x16 planes, Table 4")
     ap.add_argument("--strong", action="store_true",
@@ -679,7 +680,9 @@ def main():
     env = {"dev": dev, "dist": dist, "world": world, "rank": rank, "local_rank": local_rank, "peaks": peaks}
 
     pk = None
-    if args.cluster:
+    if args.plane_kernel is not None:
+        pk = args.plane_kernel
+    elif args.cluster:
         from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER as pk
     res = run_config(wl, args, env, do_e2e=not args.no_e2e, do_cpu=not args.no_cpu_baseline, headline=True, plane_kernel=pk)
     per_config = None

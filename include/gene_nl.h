@@ -140,6 +140,8 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
  */
 #define GENE_NL_KERNEL_AUTO 0
 #define GENE_NL_KERNEL_CLUSTER 1
+#define GENE_NL_KERNEL_GROUP 2
+#define GENE_NL_KERNEL_BATCHED 3
 int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind);
 
 /*

@@ -157,7 +157,7 @@ def gene_nl_set_scratch_bytes(h, nbytes: int) -> None:
         raise GeneNLError(f"gene_nl_set_scratch_bytes failed ({rc}): {gene_nl_last_error()}")
 
 
-GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER = 0, 1
+GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP, GENE_NL_KERNEL_BATCHED = 0, 1, 2, 3
 
 
 def gene_nl_set_plane_kernel(h, kind: int) -> None:

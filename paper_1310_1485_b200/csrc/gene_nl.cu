@@ -20,6 +20,7 @@
 #include "nl_fused.cuh"
 #include "nl_fused2.cuh"
 #include "nl_cluster.cuh"
+#include "nl_group.cuh"
 #include "nl_kernels.cuh"
 #include "nl_pipe.cuh"
 
@@ -51,10 +52,16 @@ typedef void (*fused_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cpl
 typedef void (*fused2_fn)(const cplx*, cplx*, const cplx*, const cplx*, int, int, int, int, double, double, double);
 typedef void (*cluster_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, double, double, double);
 
+typedef void (*group_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, cplx*, unsigned*, int, int, int, double,
+                         double, double);
+
 struct FusedKernel {
     fused_fn fn = nullptr;
     fused2_fn fn2 = nullptr;  // second-generation kernel (nl_fused2.cuh); used when available
     cluster_fn fnc = nullptr; // the plane spread over a thread-block cluster (nl_cluster.cuh); chi shared over v only
+    group_fn fng = nullptr;   // the plane spread over a group of co-resident CTAs, hand-overs through L2 (nl_group.cuh)
+    int group = 1;            // CTAs per group
+    size_t group_scratch = 0; // bytes of Z + P scratch per group
     int cluster = 1;          // CTAs per cluster
     size_t smem = 0;
     int nt = 0;
@@ -70,6 +77,26 @@ FusedKernel make_cluster()
     k.smem = K::SMEM_BYTES;
     k.nt = K::NT;
     return k;
+}
+
+template <int AX, int BX, int AY, int G, int NW>
+FusedKernel make_group()
+{
+    using K = gnl::Grouped<AX, BX, AY, G, NW>;
+    FusedKernel k;
+    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW>;
+    k.group = G;
+    k.group_scratch = sizeof(cplx) * K::GROUP_SCRATCH_CPLX;
+    k.smem = K::SMEM_BYTES;
+    k.nt = K::NT;
+    return k;
+}
+
+// Planes beyond one SM, chi shared over v: groups of G co-resident CTAs per plane, Z and P through L2
+bool find_group(int nx, int ny, FusedKernel* out)
+{
+    if (nx == 384 && ny == 192) { *out = make_group<24, 16, 24, 4, 8>(); return out->smem <= 227 * 1024; }
+    return false;
 }
 
 // Planes whose Z exceeds one SM but fits the shared memory of a portable cluster (8 CTAs): 384 x 192 (configs[2])
@@ -231,6 +258,8 @@ bool find_y(int ny, int nx, YKernels* out)
 
 struct Scratch {
     cplx *Z = nullptr, *P = nullptr, *R = nullptr;
+    cplx* GS = nullptr;       // group kernel: Z + P of every group's current plane (L2 resident)
+    unsigned* cnt = nullptr;  // group kernel: two hand-over counters per group
 };
 
 // Optional per-launch CUDA-event timing (gene_nl_compute_profiled): kernel classes
@@ -281,6 +310,8 @@ struct gene_nl_plan {
     XKernels xk;
     YKernels yk;
     FusedKernel fk;
+    FusedKernel gk;           // the group kernel for this plane size, if there is one
+    int gk_grid = 0;          // its grid: co-resident groups x CTAs per group
     FusedKernel ck;           // the cluster kernel for this plane size, if there is one (gene_nl_set_plane_kernel)
     int ck_grid = 0;          // its grid: resident clusters x CTAs per cluster
     FusedKernel fk_auto;      // what gene_nl_create selected
@@ -311,11 +342,12 @@ bool alloc_scratch(size_t zbytes, size_t pbytes, size_t rbytes, Scratch* s)
     if (!cuda_ok(cudaMalloc(&s->R, rbytes), "cudaMalloc(Rchi)")) return false;
     return true;
 }
-bool alloc_scratch(gene_nl_plan* h, Scratch* s) { return alloc_scratch(h->zbytes, h->pbytes, h->rbytes, s); }
+bool alloc_scratch(gene_nl_plan* h, Scratch* s);
 void free_scratch(Scratch* s)
 {
-    cudaFree(s->Z); cudaFree(s->P); cudaFree(s->R);
-    s->Z = s->P = s->R = nullptr;
+    cudaFree(s->Z); cudaFree(s->P); cudaFree(s->R); cudaFree(s->GS); cudaFree(s->cnt);
+    s->Z = s->P = s->R = s->GS = nullptr;
+    s->cnt = nullptr;
 }
 
 bool upload_twiddles(int n, cplx** out)
@@ -351,6 +383,18 @@ bool upload_const_twiddles()
 // Batching for the plan's scratch budget.  Batched path: chunk = nzb z-planes x all v; batch = nzb x nvb planes whose
 // scratch set fits the budget.  Fused path: nss (w,s) slabs per launch (their real-space chi is kept), nbz chi planes
 // per k_xinv / k_yreal batch.  Sets nzb, nvb, nss, nbz and the byte sizes of one scratch set.
+bool alloc_group_scratch(gene_nl_plan* h, Scratch* s)
+{
+    if (!h->fused || !h->fk.fng) return true;
+    const int ngroup = h->fused_grid / h->fk.group;
+    return cuda_ok(cudaMalloc(&s->GS, h->fk.group_scratch * (size_t)ngroup), "cudaMalloc(group scratch)") &&
+           cuda_ok(cudaMalloc(&s->cnt, sizeof(unsigned) * 2 * (size_t)ngroup), "cudaMalloc(group counters)");
+}
+bool alloc_scratch(gene_nl_plan* h, Scratch* s)
+{
+    return alloc_scratch(h->zbytes, h->pbytes, h->rbytes, s) && alloc_group_scratch(h, s);
+}
+
 void configure_batching(gene_nl_plan* h)
 {
     const int nz = h->nz, nv = h->nv;
@@ -505,7 +549,22 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const size_t goff = (size_t)s0 * h->nz * h->nv * h->M;
             long long T = (long long)ns * h->nz * h->nv;
             int grid = (T < h->fused_grid) ? (int)T : h->fused_grid;
-            if (h->fk.fnc) {
+            if (h->fk.fng) {
+                // cooperative launch (the CTAs of a group wait on one another); whole groups only
+                const int G = h->fk.group;
+                long long ngr = (T < h->fused_grid / G) ? T : h->fused_grid / G;
+                cudaMemsetAsync(s.cnt, 0, sizeof(unsigned) * 2 * (size_t)(h->fused_grid / G), st);
+                cudaLaunchConfig_t cfg = {};
+                cudaLaunchAttribute at[1];
+                cfg.gridDim = dim3((unsigned)(ngr * G));
+                cfg.blockDim = dim3((unsigned)h->fk.nt);
+                cfg.dynamicSmemBytes = h->fk.smem;
+                cfg.stream = st;
+                at[0].id = cudaLaunchAttributeCooperative;
+                at[0].val.cooperative = 1;
+                cfg.attrs = at; cfg.numAttrs = 1;
+                GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fng, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)h->twx, (const cplx*)h->twy, s.GS, s.cnt, h->nz, h->nv, ns, h->kxmin, h->kymin, coef)));
+            } else if (h->fk.fnc) {
                 // whole clusters only; a cluster walks planes with the stride of the cluster count
                 const int C = h->fk.cluster;
                 long long ncl = (T < h->fused_grid / C) ? T : h->fused_grid / C;
@@ -602,6 +661,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     // clusters of 8 CTAs are co-resident on the 148 SMs, and the DSMEM hand-overs run at 18 B/clk/SM in series with the
     // butterflies; DESIGN.md sect. 6e), so it is selected on request only (gene_nl_set_plane_kernel).
     if (!h->fused && !h->em && !h->chi_has_v) find_cluster(h->Nx, h->Ny, &h->ck);
+    if (!h->fused && !h->em && !h->chi_has_v) find_group(h->Nx, h->Ny, &h->gk);
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -615,6 +675,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
               set_smem(h->xk.inv, h->xk.smem_inv, "k_xinv smem") && set_smem(h->xk.fwd, h->xk.smem_fwd, "k_xfwd smem") &&
               set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
               (!h->ck.fnc || set_smem(h->ck.fnc, h->ck.smem, "k_plane_cluster smem")) &&
+              (!h->gk.fng || set_smem(h->gk.fng, h->gk.smem, "k_plane_group smem")) &&
               (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
                                        : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
               upload_const_twiddles();
@@ -635,6 +696,18 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             h->ck = FusedKernel();   // no cluster of that size fits this device: the option is not offered
         } else {
             h->ck_grid = ncl * h->ck.cluster;
+        }
+    }
+    if (ok && h->gk.fng) {  // co-resident groups (cooperative launch)
+        int sms = 0, occ = 0, coop = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->gk.fng, h->gk.nt, h->gk.smem) != cudaSuccess || occ < 1 ||
+            sms < h->gk.group) {
+            cudaGetLastError();
+            h->gk = FusedKernel();
+        } else {
+            h->gk_grid = (sms / h->gk.group) * h->gk.group;
         }
     }
     h->fk_auto = h->fk; h->fused_auto = h->fused; h->fused_grid_auto = h->fused_grid;
@@ -741,7 +814,15 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
-    if (kind != GENE_NL_KERNEL_AUTO && kind != GENE_NL_KERNEL_CLUSTER) { set_err("gene_nl_set_plane_kernel: unknown kind"); return GENE_NL_EINVAL; }
+    if (kind != GENE_NL_KERNEL_AUTO && kind != GENE_NL_KERNEL_CLUSTER && kind != GENE_NL_KERNEL_GROUP && kind != GENE_NL_KERNEL_BATCHED) {
+        set_err("gene_nl_set_plane_kernel: unknown kind");
+        return GENE_NL_EINVAL;
+    }
+    if (kind == GENE_NL_KERNEL_GROUP && !h->gk.fng) {
+        set_err("gene_nl_set_plane_kernel: no group kernel for this plan (384 x 192 padded grid, chi shared over v, cooperative launch)");
+        return GENE_NL_EUNSUPPORTED;
+    }
+    if (kind == GENE_NL_KERNEL_BATCHED && h->em) kind = GENE_NL_KERNEL_AUTO;
     if (kind == GENE_NL_KERNEL_CLUSTER && !h->ck.fnc) {
         set_err("gene_nl_set_plane_kernel: no cluster kernel for this plan (384 x 192 padded grid, chi shared over v, a device that keeps clusters of 8 CTAs resident)");
         return GENE_NL_EUNSUPPORTED;
@@ -751,6 +832,8 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
     free_stages(h);
     free_scratch(&h->scr);
     if (kind == GENE_NL_KERNEL_CLUSTER) { h->fk = h->ck; h->fused = true; h->fused_grid = h->ck_grid; }
+    else if (kind == GENE_NL_KERNEL_GROUP) { h->fk = h->gk; h->fused = true; h->fused_grid = h->gk_grid; }
+    else if (kind == GENE_NL_KERNEL_BATCHED) { h->fk = FusedKernel(); h->fused = false; h->fused_grid = 0; }
     else { h->fk = h->fk_auto; h->fused = h->fused_auto; h->fused_grid = h->fused_grid_auto; }
     configure_batching(h);
     if (!alloc_scratch(h, &h->scr)) { free_scratch(&h->scr); return GENE_NL_ENOMEM; }
@@ -880,7 +963,7 @@ static int host_impl(gene_nl_plan* h, const void* chi_, const void* apar_, const
                  cuda_ok(cudaMalloc(&s.rhs, slab_g), "cudaMalloc(stage rhs)") &&
                  cuda_ok(cudaMalloc(&s.chi, slab_c), "cudaMalloc(stage chi)") &&
                  (!h->em || cuda_ok(cudaMalloc(&s.apar, slab_c), "cudaMalloc(stage A_par)")) &&
-                 alloc_scratch(h->zbytes, h->pbytes, rbytes1, &s.scr);
+                 alloc_scratch(h->zbytes, h->pbytes, rbytes1, &s.scr) && alloc_group_scratch(h, &s.scr);
             if (!ok) break;
         }
         if (!ok) {
@@ -975,7 +1058,7 @@ double gene_nl_query(const gene_nl_plan* h, int what)
     case 4: return h->fused ? (double)((h->nw * h->nspec + h->nss - 1) / h->nss)
                             : (double)h->nw * h->nspec * chunks_per_slab(h) * ((h->nv + h->nvb - 1) / h->nvb);
     case 7: return h->fused ? 1.0 : 0.0;
-    case 8: return h->fk.fnc ? 1.0 : 0.0;
+    case 8: return h->fk.fnc ? 1.0 : (h->fk.fng ? 2.0 : 0.0);
     case 5: return 16.0 * M * (3.0 + c);
     case 6: {
         const double t2d = h->nky0 * 5.0 * Nx * std::log2(Nx) + Nx * 2.5 * Ny * std::log2(Ny);

@@ -1,0 +1,401 @@
+// nl_group.cuh -- the fused per-plane kernel for planes beyond one SM, spread over a GROUP of G co-resident CTAs whose
+// x<->y hand-overs go through a small per-group scratch that lives in the 126 MB L2.
+//
+// Same steps and the same phase structure as nl_cluster.cuh, changed where the
+// measurements of that kernel pointed (DESIGN.md sect. 6e): distributed-shared-memory stores run at 18 B/clk/SM, in
+// series with the butterflies, and only 15 clusters of 8 CTAs are co-resident on the 148 SMs.  Here
+//   * a group is G consecutive CTAs of one cooperative launch (any G that divides the work; no placement constraint,
+//     every SM is used), one plane per group at a time;
+//   * the half-transformed arrays Z[pair][m+Nx/2 | m][cc] and P[pair][cc] of the group's CURRENT plane sit in global
+//     memory, 1.1 MB per group at 384 x 192: written and read again within microseconds and overwritten by the next
+//     plane, so the lines never leave L2 (HBM sees g, rhs and the chi rows only);
+//   * rows come back for the y transforms as ONE 1-D bulk copy (TMA, cp.async.bulk + mbarrier) per row pair, straight
+//     into the warp's pair storage; g column blocks come in the same way, a block ahead;
+//   * the two hand-overs of a plane are ordered by two counters per group in global memory (release: bar.sync +
+//     __threadfence + atomicAdd by one thread; acquire: one thread polls, bar.sync), monotonic over the launch.
+// Phases per plane and CTA r of the group (Nx = AX * BX, Ny = 8 AY):
+//   X1  column units u = r, r + G, ... (8 stored columns each): derivative, pad, pruned radix-AX, radix-BX, rows to Z
+//   Y   row pairs [r PPG, (r+1) PPG): a warp takes NPW pairs at a time and runs, with __syncwarp only, pruned radix-AY +
+//       radix-8 to real space (rows m, then rows m + Nx/2, one exchange tile per pair behind its rows), the bracket
+//       with the chi rows, radix-8 + pruned-output radix-AY back; P rows go to global memory from registers
+//   X2  column units again: unpack the row pair, radix-BX, pruned-output radix-AX, delete modes, prefactor, rhs +=
+// Scratch reads bypass L1 (ld.global.cg / TMA): L1 is not coherent across SMs and the addresses repeat every plane.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "nl_cluster.cuh"
+
+namespace gnl {
+
+__device__ __forceinline__ cplx ldg_cg(const cplx* p)   // L2 only
+{
+    cplx v;
+    asm volatile("ld.global.cg.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+template <int AX_, int BX_, int AY_, int G_, int NW_>
+struct Grouped {
+    static constexpr int AX = AX_, BX = BX_, AY = AY_, G = G_, NW = NW_;
+    static constexpr int NX = AX * BX, NY = 8 * AY, C2 = BX / 2;
+    static constexpr int NKY0 = NY / 3, W2 = 2 * NKY0, NPAIR = NX / 2;
+    static constexpr int M = NX / 3, NX0 = 2 * M;
+    static constexpr int CK = 8;                       // stored columns per unit: 128 B runs in both hand-overs
+    static constexpr int NUNIT = NKY0 / CK;            // column units per plane
+    static constexpr int PPG = NPAIR / G;              // row pairs per CTA
+    static constexpr int NPW = 3;                      // row pairs per warp item
+    static constexpr int NITEM = PPG / NPW;            // items per CTA
+    static constexpr int NT = 32 * NW;
+    static constexpr int FY = AY * 9;                  // y exchange tile of one row: [k1][9]
+    static constexpr int PS = (W2 + FY) | 1;           // pair storage: rows m + NX/2 | m, the tile over row m and beyond
+    static constexpr int YB_CPLX = NW * NPW * PS;
+    static constexpr int BPX = Tile<AX, BX>::BP, AXH = AX / 2;
+    static constexpr int CSH = ((AXH * BPX) | 1) + ((((AXH * BPX) | 1) % 8 == 1) ? 4 : 0);   // half-k1 tile of one column-sign
+    static constexpr int E_CPLX = 2 * CK * CSH;        // X1: both signs of a unit's columns, half of the k1 range at a time
+    static constexpr int CSF = Tile<AX, BX>::STRIDE;
+    static constexpr int TX_CPLX = CK * CSF;           // X2: exchange tile of a unit's columns
+    static constexpr int XR_CPLX = E_CPLX > TX_CPLX ? E_CPLX : TX_CPLX;
+    static constexpr int A_CPLX = YB_CPLX > XR_CPLX ? YB_CPLX : XR_CPLX;   // the x tiles and the y pair storages share a region
+    static constexpr int G_CPLX = CK * NX0;            // one unit's columns of a g plane (one contiguous block)
+    static constexpr int TWX = AX * BPX, TWY = AY * 9;
+    static constexpr int NBAR = 1 + NW;                // mbarriers: g block, rows of each warp
+    static constexpr int SMEM_CPLX = A_CPLX + G_CPLX + TWX + TWY + (NBAR + 1) / 2;
+    static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
+    static constexpr size_t ZS_CPLX = (size_t)NPAIR * 2 * W2, PS_CPLX = (size_t)NPAIR * W2;   // per-group scratch
+    static constexpr size_t GROUP_SCRATCH_CPLX = ZS_CPLX + PS_CPLX;
+    static_assert(AX % 3 == 0 && AY % 3 == 0 && AX % 2 == 0 && BX % 2 == 0, "3/2 rule; half-k1 tiles; row pairs");
+    static_assert(NKY0 % CK == 0 && NUNIT % G == 0 && NPAIR % G == 0 && PPG % NPW == 0, "the group divides the work");
+    static_assert(NPW * 8 <= 32 && AY <= 32 && NKY0 == 8 * (AY / 3), "lanes of the y stages");
+    static_assert(2 * CK * BX == NT && (2 * CK * AXH) % 32 == 0 && 2 * CK * AXH <= NT && CK * AX <= NT && CK * BX <= NT,
+                  "one item per thread in every x stage");
+};
+
+// grid = groups * G CTAs (cooperative launch: every CTA is resident).  scratch: groups * GROUP_SCRATCH_CPLX values;
+// cnt: 2 * groups counters, zeroed before the launch.
+template <int AX, int BX, int AY, int G, int NW>
+__global__ void __launch_bounds__(32 * NW, 1)
+k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R,
+              const cplx* __restrict__ twx_g, const cplx* __restrict__ twy_g, cplx* __restrict__ scratch,
+              unsigned* __restrict__ cnt, int nz, int nv, int nslab, double kxmin, double kymin, double coef)
+{
+    using K = Grouped<AX, BX, AY, G, NW>;
+    constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR;
+    constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT;
+    constexpr int PS = K::PS, BPX = K::BPX, CSH = K::CSH, CSF = K::CSF, AXH = K::AXH;
+    constexpr int AX1 = AX / 3, AY1 = AY / 3;
+    constexpr unsigned FULL = 0xffffffffu;
+    constexpr uint32_t GBYTES = (uint32_t)(K::G_CPLX * sizeof(cplx));
+
+    extern __shared__ cplx smem[];
+    cplx* A = smem;                        // X1: E / X2: Tx / Y: pair storages of the warps
+    cplx* Gs = A + K::A_CPLX;              // a unit's columns of g (bulk copy)
+    cplx* twx = Gs + K::G_CPLX;            // W_NX^{n2 k1}, [k1][BPX]
+    cplx* twy = twx + K::TWX;              // W_NY^{k1 k2}, [k1][9]
+    const uint32_t bars = smem_u32(twy + K::TWY);
+    const uint32_t gbar = bars;
+
+    const int tid = threadIdx.x;
+    const int lane0 = tid & 31;
+    const int warp = __shfl_sync(FULL, tid >> 5, 0);
+    const uint32_t ybar = bars + 8 + 8 * (uint32_t)warp;
+    const int ngroup = gridDim.x / G, grp = blockIdx.x / G, rank = blockIdx.x % G;
+    cplx* Zs = scratch + (size_t)grp * K::GROUP_SCRATCH_CPLX;   // [pair][row m + NX/2 | row m][cc]
+    cplx* Ps = Zs + K::ZS_CPLX;                                 // [pair][cc]
+    unsigned* zcnt = cnt + 2 * grp;
+    unsigned* pcnt = zcnt + 1;
+
+    load_twiddles_ab<AX, BX>(twx, twx_g);
+    load_twiddles_ab<AY, 8>(twy, twy_g);
+    if (tid == 0) {
+        mbar_init(gbar, 1);
+        for (int w = 0; w < NW; ++w) mbar_init(bars + 8 + 8 * w, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const unsigned T = (unsigned)nslab * (unsigned)nz * (unsigned)nv;   // planes of this launch (< 2^31: checked by the host)
+    const size_t plane_elems = (size_t)NX0 * NKY0;
+    // planes are walked v-fastest so that neighbouring groups share a chi plane in L2
+    auto plane_of = [&](unsigned tt) {
+        const unsigned v = tt % (unsigned)nv, zs = tt / (unsigned)nv;
+        const unsigned z = zs % (unsigned)nz, sl = zs / (unsigned)nz;
+        return (size_t)z + (size_t)nz * ((size_t)v + (size_t)nv * sl);
+    };
+    auto request_g = [&](unsigned tt, int unit) {   // one thread: columns [8 unit, 8 unit + 8) of plane tt -> Gs
+        mbar_arrive_expect_tx(gbar, GBYTES);
+        bulk_g2s(smem_u32(Gs), g + plane_of(tt) * plane_elems + (size_t)unit * CK * NX0, GBYTES, gbar);
+    };
+    if (tid == 0 && (unsigned)grp < T) request_g((unsigned)grp, rank);
+
+    uint32_t gph = 0, yph = 0;
+    unsigned it = 0;
+    for (unsigned t = (unsigned)grp; t < T; t += (unsigned)ngroup, ++it) {
+        const size_t p = plane_of(t);
+        const size_t q = (size_t)((t / (unsigned)nv) % (unsigned)nz) + (size_t)nz * (size_t)(t / ((unsigned)nv * (unsigned)nz));
+        cplx* Rb = rhs + p * plane_elems;
+        const cplx* Rc = R + q * ((size_t)NX * NY);
+
+        // =============== X1: derivative, pad, x-synthesis of this CTA's column units; rows go to Z ===============
+#pragma unroll 1
+        for (int unit = rank; unit < K::NUNIT; unit += G) {
+            mbar_wait(gbar, gph);
+            gph ^= 1;
+            if (unit == 0) {   // Hermitian part of the ky = 0 column (reading R7), in place in the staged block
+                if (tid > 0 && tid < NX0 / 2) {
+                    const cplx a = Gs[tid], b = Gs[NX0 - tid];
+                    Gs[tid] = cmake(0.5 * (a.x + b.x), 0.5 * (a.y - b.y));
+                    Gs[NX0 - tid] = cmake(0.5 * (a.x + b.x), 0.5 * (b.y - a.y));
+                } else if (tid == 0) {
+                    Gs[0].y = 0.0;
+                }
+                __syncthreads();
+            }
+            // stage 1, every thread: column-sign c2 = (sign, column), position n2: pruned radix-AX over n1 (i = n2 + BX n1),
+            // twiddle W_NX^{n2 k1}.  The k1 < AX/2 half goes to E now, the other half after the first stage-2 pass.
+            const int n2 = opaque(tid % BX), c2 = opaque(tid / BX);
+            cplx out[AX];
+            {
+                const int col1 = c2 % CK;
+                const cplx* Fc = Gs + col1 * NX0 + n2;
+                const double ky = kymin * (double)(unit * CK + col1), dn2 = (double)n2;
+                const double kys = (c2 / CK) ? ky : -ky;  // (i kx - ky) F for +ky, (i kx + ky) F for -ky
+                cplx lo[AX1], hi[AX1];
+#pragma unroll
+                for (int a = 0; a < AX1; ++a) {
+                    lo[a] = deriv_mul(Fc[BX * a], kxmin * (dn2 + (double)(BX * a)), kys);                // i = n2 + BX a      (kx >= 0)
+                    hi[a] = deriv_mul(Fc[BX * a + M], kxmin * (dn2 + (double)(BX * a + M - NX0)), kys);  // i = n2 + BX a + M  (kx < 0)
+                }
+                if (n2 == 0) hi[0] = cmake(0.0, 0.0);  // i = M: the Nyquist row is ignored (R6)
+                dft_pruned_in<AX, +1>(lo, hi, out);
+#pragma unroll
+                for (int k1 = 1; k1 < AX; ++k1) {
+                    const cplx w = twx[k1 * BPX + n2];
+                    out[k1] = cmul(out[k1], w.x, w.y);
+                }
+            }
+            __syncthreads();   // every thread has read its g values
+            if (tid == 0) {    // the next block: this CTA's next unit of this plane, or its first unit of the next plane
+                if (unit + G < K::NUNIT) request_g(t, unit + G);
+                else if (t + (unsigned)ngroup < T) request_g(t + (unsigned)ngroup, rank);
+            }
+#pragma unroll
+            for (int hk = 0; hk < 2; ++hk) {
+                {
+                    cplx* Ec = A + c2 * CSH + n2;
+#pragma unroll
+                    for (int k1 = 0; k1 < AXH; ++k1) Ec[k1 * BPX] = out[hk * AXH + k1];
+                }
+                __syncthreads();
+                if (tid < 2 * CK * AXH) {
+                    // stage 2: radix-BX over n2 for fixed k1; row m = k1 + AX k2 is half k2 / C2 of pair k1 + AX (k2 mod C2).
+                    // Lanes run over the 2 CK column-signs: two 128 B runs per store instruction and k1 value.
+                    const int c2s = tid % (2 * CK), k1 = hk * AXH + tid / (2 * CK);
+                    const int sg = c2s / CK, kyi = unit * CK + c2s % CK;
+                    const bool zero = (sg == 1 && kyi == 0);  // there is no -0 column: slot cc = nky0 holds zeros
+                    cplx v[BX];
+                    const cplx* Ec = A + c2s * CSH + (k1 - hk * AXH) * BPX;
+#pragma unroll
+                    for (int i = 0; i < BX; ++i) v[i] = zero ? cmake(0.0, 0.0) : Ec[i];
+                    Dft<BX, +1>::run(v);
+                    const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
+                    cplx* Zc = Zs + (size_t)k1 * (2 * W2) + cc;
+                    const double sgn = sg ? -1.0 : 1.0;   // -ky columns hold the conjugate
+#pragma unroll
+                    for (int k2 = 0; k2 < BX; ++k2)      // pair storage: row m + NX/2 (k2 >= C2) first, then row m
+                        Zc[(size_t)(AX * (k2 % C2)) * (2 * W2) + (k2 < C2 ? W2 : 0)] = cmake(v[k2].x, sgn * v[k2].y);
+                }
+                __syncthreads();  // E is free for the second half / the next unit
+            }
+        }
+        // ---- hand-over 1: every CTA of the group has written its columns of Z ----
+        if (tid == 0) {
+            __threadfence();
+            atomicAdd(zcnt, 1u);
+            while (ld_acquire_gpu(zcnt) < (unsigned)G * (it + 1)) {}
+        }
+        __syncthreads();
+
+        // =============== Y: this CTA's row pairs, a warp takes NPW of them at a time, __syncwarp only ===============
+        {
+            const int lane = opaque(lane0);
+            const int k1y = lane < AY ? lane : lane - AY;   // lanes >= AY shadow an item (same addresses) and skip the stores
+            const bool act2 = lane < AY;
+            const int j1 = (lane >> 3) < NPW ? (lane >> 3) : 0;   // Y1 / Y3 item: pair j1 of the warp item, position lane & 7
+            const bool act1 = (lane >> 3) < NPW;
+            const int n2 = lane & 7;
+            cplx* Zw = A + (warp * NPW) * PS;                     // this warp's pair storages
+            cplx tq[8];
+#pragma unroll
+            for (int k2 = 1; k2 < 8; ++k2) tq[k2] = twy[k1y * 9 + k2];
+#pragma unroll 1
+            for (int item = warp; item < K::NITEM; item += NW) {
+                const int q0 = rank * PPG + item * NPW;           // first pair of the item
+                if (lane == 0) {   // the rows of the item's pairs: one bulk copy per pair (2 W2 values, contiguous in Z)
+                    fence_proxy_async();
+                    mbar_arrive_expect_tx(ybar, (uint32_t)(NPW * 2 * W2 * sizeof(cplx)));
+#pragma unroll
+                    for (int j = 0; j < NPW; ++j)
+                        bulk_g2s(smem_u32(Zw + j * PS), Zs + (size_t)(q0 + j) * (2 * W2), (uint32_t)(2 * W2 * sizeof(cplx)), ybar);
+                }
+                cplx chv[8];
+                {
+                    const cplx* Rr = Rc + (size_t)q0 * NY + k1y;
+#pragma unroll
+                    for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
+                }
+                mbar_wait(ybar, yph);
+                yph ^= 1;
+                double nlx[NPW][8];                                   // bracket of the rows m (first halves), kept in registers
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    {  // Y1: pruned radix-AY of rows m (h = 0: second half of the storage) / m + NX/2 (h = 1: first half)
+                        const cplx* Zr = Zw + j1 * PS + (h ? 0 : W2) + n2;
+                        cplx lo[AY1], hi[AY1];
+#pragma unroll
+                        for (int a = 0; a < AY1; ++a) {
+                            lo[a] = Zr[8 * a];
+                            hi[a] = Zr[8 * a + NKY0];
+                        }
+                        cplx out[AY];
+                        dft_pruned_in<AY, +1>(lo, hi, out);
+                        __syncwarp(FULL);  // h = 0: rows m are in registers before the tiles overwrite them; h = 1: Y2 done
+                        if (act1) {
+                            cplx* tile = Zw + j1 * PS + W2 + n2;
+#pragma unroll
+                            for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
+                        }
+                    }
+                    __syncwarp(FULL);
+#pragma unroll
+                    for (int j = 0; j < NPW; ++j) {  // Y2: twiddle + radix-8 to real space, bracket; pair j, k1 = lane
+                        // chi rows of the NEXT row (pair j+1 of this half, or pair 0 of the second half), requested before
+                        // this row's butterflies so that their latency hides behind them
+                        cplx chn[8];
+                        const int jn = (j + 1 < NPW) ? j + 1 : 0, hn = (j + 1 < NPW) ? h : 1;
+                        if (!(h == 1 && j + 1 == NPW)) {
+                            const cplx* Rr = Rc + (size_t)(q0 + jn + hn * NPAIR) * NY + k1y;
+#pragma unroll
+                            for (int k2 = 0; k2 < 8; ++k2) chn[k2] = ldg_nc_early(Rr + AY * k2);
+                        }
+                        cplx* tile = Zw + j * PS + W2 + k1y * 9;
+                        cplx v[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) v[i] = tile[i];
+                        dft8_twiddled<+1>(v, tq);   // (dx g + i dy g)(row, y = k1 + AY k2)
+                        if (h == 0) {
+#pragma unroll
+                            for (int k2 = 0; k2 < 8; ++k2) nlx[j][k2] = fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x);
+                        } else {
+                            cplx w[8];
+#pragma unroll
+                            for (int k2 = 0; k2 < 8; ++k2)
+                                w[k2] = cmake(nlx[j][k2], fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x));
+                            Dft<8, -1>::run(w);
+#pragma unroll
+                            for (int k2 = 1; k2 < 8; ++k2) w[k2] = cmul(w[k2], tq[k2].x, -tq[k2].y);
+                            if (act2) {  // own slots of the tile: no other lane reads or writes them in this phase
+#pragma unroll
+                                for (int k2 = 0; k2 < 8; ++k2) tile[k2] = w[k2];
+                            }
+                        }
+                        if (!(h == 1 && j + 1 == NPW)) {
+#pragma unroll
+                            for (int k2 = 0; k2 < 8; ++k2) chv[k2] = chn[k2];
+                        }
+                    }
+                    __syncwarp(FULL);
+                }
+                {  // Y3: pruned-output radix-AY; P[pair][cc] goes to global memory (L2), 128 B runs
+                    const cplx* tile = Zw + j1 * PS + W2 + n2;
+                    cplx in[AY];
+#pragma unroll
+                    for (int n1 = 0; n1 < AY; ++n1) in[n1] = tile[n1 * 9];
+                    cplx lo[AY1], hi[AY1];
+                    dft_pruned_out<AY, -1>(in, lo, hi);
+                    if (act1) {
+                        cplx* Pp = Ps + (size_t)(q0 + j1) * W2 + n2;
+#pragma unroll
+                        for (int c = 0; c < AY1; ++c) {
+                            Pp[8 * c] = lo[c];          // +ky half: cc = ky = n2 + 8 c
+                            Pp[8 * c + NKY0] = hi[c];   // -ky half: cc = nky0 + n2 + 8 c  <->  ky = nky0 - n2 - 8 c
+                        }
+                    }
+                }
+                __syncwarp(FULL);   // the tiles are consumed before the next item's rows land on them
+            }
+        }
+        // ---- hand-over 2: every CTA of the group has written its rows of P ----
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            atomicAdd(pcnt, 1u);
+            while (ld_acquire_gpu(pcnt) < (unsigned)G * (it + 1)) {}
+        }
+        __syncthreads();
+
+        // =============== X2: x-analysis of this CTA's column units; delete modes, prefactor, add ===============
+#pragma unroll 1
+        for (int unit = rank; unit < K::NUNIT; unit += G) {
+            // rhs values of this thread's share of stage 2, requested ahead of stage 1
+            cplx r0[AX1], r1[AX1];
+            const int k2s = tid % BX, cols = (tid / BX) % CK;
+            if (tid < CK * BX) {
+                const cplx* Rcol = Rb + (size_t)(unit * CK + cols) * NX0 + k2s;
+#pragma unroll
+                for (int c = 0; c < AX1; ++c) {
+                    r0[c] = ldg_early(Rcol + BX * c);
+                    r1[c] = ldg_early(Rcol + BX * c + M);
+                }
+            }
+            if (tid < CK * AX) {  // stage 1: unpack the row pair, radix-BX over n2 for fixed n1 (m = n1 + AX n2), twiddle
+                const int col = tid % CK, n1 = tid / CK;
+                const int kyi = unit * CK + col;
+                const int ccm = kyi ? W2 - kyi : 0;
+                cplx x[BX];
+#pragma unroll
+                for (int i = 0; i < C2; ++i) {
+                    const cplx* Pr = Ps + (size_t)(n1 + AX * i) * W2;
+                    const cplx pp = ldg_cg(Pr + kyi), pm = ldg_cg(Pr + ccm);
+                    x[i] = cmake(pp.x + pm.x, pp.y - pm.y);          // 2 N^_m  = P+ + conj P-
+                    x[i + C2] = cmake(pp.y + pm.y, pm.x - pp.x);     // 2 N^_m' = -i (P+ - conj P-)
+                }
+                Dft<BX, -1>::run(x);
+                cplx* Ec = A + col * CSF + n1 * BPX;
+#pragma unroll
+                for (int k2 = 0; k2 < BX; ++k2) {
+                    const cplx w = twx[n1 * BPX + k2];
+                    Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], w.x, -w.y);
+                }
+            }
+            __syncthreads();
+            if (tid < CK * BX) {  // stage 2: pruned-output radix-AX over n1 for fixed k2; i = k2 + BX c
+                const int k2 = k2s, col = cols;
+                cplx in[AX];
+                const cplx* Ec = A + col * CSF + k2;
+#pragma unroll
+                for (int n1 = 0; n1 < AX; ++n1) in[n1] = Ec[n1 * BPX];
+                cplx lo[AX1], hi[AX1];
+                dft_pruned_out<AX, -1>(in, lo, hi);
+                cplx* Rcol = Rb + (size_t)(unit * CK + col) * NX0 + k2;
+#pragma unroll
+                for (int c = 0; c < AX1; ++c) {
+                    Rcol[BX * c] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));
+                    if (c != 0 || k2 != 0)  // i = M is the Nyquist row: untouched (R6)
+                        Rcol[BX * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
+                }
+            }
+            __syncthreads();  // the tile is consumed before the next unit / the next plane's E overwrites it
+        }
+    }
+}
+
+}  // namespace gnl

@@ -190,54 +190,64 @@ def test_plane_sharded_ranks_assemble_to_the_unsharded_result(cuda_device, world
         assert torch.equal(torch.cat(parts), whole.reshape(-1))
 
 
-# ---- the cluster kernel (gene_nl_set_plane_kernel(GENE_NL_KERNEL_CLUSTER)): 384 x 192 planes over 8 CTAs, DSMEM hand-overs ----
-CLUSTER_SHAPES = [(256, 64, 1, 1, 1, 1),       # one plane: one cluster busy, the others idle
-                  (256, 64, 2, 3, 1, 1),
-                  (256, 64, 3, 5, 2, 2),       # 60 planes: several planes per cluster, chi shared by 5 planes
-                  (256, 64, 36, 2, 1, 1)]
+# ---- the kernels for planes beyond one SM that keep Z and P out of HBM (gene_nl_set_plane_kernel): 384 x 192 planes over a
+# cluster of 8 CTAs with DSMEM hand-overs (1), or over a group of 4 co-resident CTAs with hand-overs through L2 (2) ----
+SPREAD_SHAPES = [(256, 64, 1, 1, 1, 1),       # one plane: one cluster / group busy, the others idle
+                 (256, 64, 2, 3, 1, 1),
+                 (256, 64, 3, 5, 2, 2),       # 60 planes: several planes per cluster / group, chi shared by 5 planes
+                 (256, 64, 36, 2, 1, 1)]
+SPREAD_KINDS = [1, 2]                         # GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP
 
 
-@pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec", CLUSTER_SHAPES)
-def test_cluster_kernel_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, nw, nspec):
-    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER, GeneNL
+@pytest.mark.parametrize("kind", SPREAD_KINDS)
+@pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec", SPREAD_SHAPES)
+def test_spread_kernels_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, nw, nspec, kind):
+    from paper_1310_1485_b200 import GeneNL
     wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, False, seed=300 + nz + nv)
-    with GeneNL(wl, plane_kernel=GENE_NL_KERNEL_CLUSTER) as nl:
-        assert nl.query(7) == 1.0 and nl.query(8) == 1.0         # the cluster kernel is the one that runs
-    check_parity(wl, cuda_device, plane_kernel=GENE_NL_KERNEL_CLUSTER)
-    check_parity(wl, cuda_device, plane_kernel=GENE_NL_KERNEL_CLUSTER, scratch_bytes=20 << 20)   # several launches
-    check_parity(wl, cuda_device, plane_kernel=GENE_NL_KERNEL_CLUSTER, host=True)                 # behind the streaming driver
+    with GeneNL(wl, plane_kernel=kind) as nl:
+        assert nl.query(7) == 1.0 and nl.query(8) == float(kind)   # the requested kernel is the one that runs
+    check_parity(wl, cuda_device, plane_kernel=kind)
+    check_parity(wl, cuda_device, plane_kernel=kind, scratch_bytes=20 << 20)   # several launches
+    check_parity(wl, cuda_device, plane_kernel=kind, host=True)                 # behind the streaming driver
 
 
-def test_cluster_kernel_config2_full_size_all_planes(cuda_device):
-    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER
-    _full_size(cuda_device, 2, None, plane_kernel=GENE_NL_KERNEL_CLUSTER)
+@pytest.mark.parametrize("kind", SPREAD_KINDS)
+def test_spread_kernels_config2_full_size_all_planes(cuda_device, kind):
+    _full_size(cuda_device, 2, None, plane_kernel=kind)
 
 
-def test_cluster_kernel_properties_and_selection(cuda_device):
-    from paper_1310_1485_b200 import (GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER, GeneNL, GeneNLError,
-                                      gene_nl_set_plane_kernel)
+@pytest.mark.parametrize("kind", SPREAD_KINDS)
+def test_spread_kernels_properties_and_selection(cuda_device, kind):
+    from paper_1310_1485_b200 import (GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_BATCHED, GENE_NL_KERNEL_CLUSTER, GeneNL,
+                                      GeneNLError, gene_nl_set_plane_kernel)
+    GENE_NL_KERNEL_CLUSTER = kind   # noqa: N806  (the body below is written for "the selected kind")
     wl = W.small_workload(256, 64, 2, 3, 1, 2, 0.05, 0.05, False, seed=61)
     chi, g, rhs = W.make_inputs(wl, cuda_device)
     kw = dict(plane_kernel=GENE_NL_KERNEL_CLUSTER)
     assert torch.equal(gpu_compute(wl, chi, g, rhs, scale=0.0, **kw), rhs)          # scale = 0: bit-identical
     a = gpu_compute(wl, chi, g, rhs, **kw)
     assert torch.equal(a, gpu_compute(wl, chi, g, rhs, **kw))                       # deterministic
-    b = gpu_compute(wl, chi, g, rhs)                                                # the batched kernels (default)
+    b = gpu_compute(wl, chi, g, rhs, plane_kernel=GENE_NL_KERNEL_BATCHED)           # the batched kernels
     assert (a - b).abs().max() <= 1e-13 * (b - rhs).abs().max()
     h = wl.nx0 // 2
     assert torch.equal(W.as_planes(a, wl)[:, :, h], W.as_planes(rhs, wl)[:, :, h])  # Nyquist row untouched
     with GeneNL(wl) as nl:                                                          # switching back and forth on one plan
-        assert nl.query(8) == 0.0
         gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_CLUSTER)
         out = rhs.clone()
         nl.compute(chi, g, out)
         torch.cuda.synchronize()
         assert torch.equal(out, a)
-        gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_AUTO)
+        gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_BATCHED)
+        assert nl.query(7) == 0.0 and nl.query(8) == 0.0
         out = rhs.clone()
         nl.compute(chi, g, out)
         torch.cuda.synchronize()
         assert torch.equal(out, b)
+        gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_AUTO)
+        out = rhs.clone()
+        nl.compute(chi, g, out)
+        torch.cuda.synchronize()
+        assert (out - b).abs().max() <= 1e-13 * (b - rhs).abs().max()
         with pytest.raises(GeneNLError):
             gene_nl_set_plane_kernel(nl.h, 7)
     for bad in (W.small_workload(128, 32, 1, 1, 1, 1), W.small_workload(256, 64, 1, 1, 1, 1, chi_has_v=True)):
@@ -265,10 +275,11 @@ def test_compute_is_capturable_in_a_cuda_graph(cuda_device):
     """gene_nl_compute only enqueues kernels on the caller's stream (no synchronisation, no allocation): it can be
     captured into a CUDA graph and replayed; fused and batched paths."""
     from paper_1310_1485_b200 import GeneNL
-    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER
+    from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP
     for wl, pk in ((W.small_workload(128, 32, 2, 3, 1, 1, 0.05, 0.05, False, seed=41), None),     # fused kernel
                    (W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, True, seed=42), None),      # batched kernels
-                   (W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, False, seed=43), GENE_NL_KERNEL_CLUSTER)):
+                   (W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, False, seed=43), GENE_NL_KERNEL_CLUSTER),
+                   (W.small_workload(256, 64, 2, 2, 1, 2, 0.05, 0.05, False, seed=44), GENE_NL_KERNEL_GROUP)):
         chi, g, rhs = W.make_inputs(wl, cuda_device)
         expect = gpu_compute(wl, chi, g, rhs, plane_kernel=pk)
         out = rhs.clone()
