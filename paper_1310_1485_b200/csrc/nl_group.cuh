@@ -51,6 +51,7 @@ struct Grouped {
     static constexpr int M = NX / 3, NX0 = 2 * M;
     static constexpr int CK = 8;                       // stored columns per unit: 128 B runs in both hand-overs
     static constexpr int NUNIT = NKY0 / CK;            // column units per plane
+    static constexpr int UPC = NUNIT / G_;             // column units per CTA
     static constexpr int PPG = NPAIR / G;              // row pairs per CTA
     static constexpr int NPW = 3;                      // row pairs per warp item
     static constexpr int NITEM = PPG / NPW;            // items per CTA
@@ -62,7 +63,7 @@ struct Grouped {
     static constexpr int CSH = ((AXH * BPX) | 1) + ((((AXH * BPX) | 1) % 8 == 1) ? 4 : 0);   // half-k1 tile of one column-sign
     static constexpr int E_CPLX = 2 * CK * CSH;        // X1: both signs of a unit's columns, half of the k1 range at a time
     static constexpr int CSF = Tile<AX, BX>::STRIDE;
-    static constexpr int TX_CPLX = CK * CSF;           // X2: exchange tile of a unit's columns
+    static constexpr int TX_CPLX = (32 * NW_ / (CK * BX_)) * CK * CSF;   // X2: exchange tiles of the units of one pass
     static constexpr int XR_CPLX = E_CPLX > TX_CPLX ? E_CPLX : TX_CPLX;
     static constexpr int A_CPLX = YB_CPLX > XR_CPLX ? YB_CPLX : XR_CPLX;   // the x tiles and the y pair storages share a region
     static constexpr int G_CPLX = CK * NX0;            // one unit's columns of a g plane (one contiguous block)
@@ -77,6 +78,7 @@ struct Grouped {
     static_assert(NPW * 8 <= 32 && AY <= 32 && NKY0 == 8 * (AY / 3), "lanes of the y stages");
     static_assert(2 * CK * BX == NT && (2 * CK * AXH) % 32 == 0 && 2 * CK * AXH <= NT && CK * AX <= NT && CK * BX <= NT,
                   "one item per thread in every x stage");
+    static_assert(UPC % (NT / (CK * BX)) == 0, "X2 takes NT / (CK BX) units per pass");
 };
 
 // grid = groups * G CTAs (cooperative launch: every CTA is resident).  scratch: groups * GROUP_SCRATCH_CPLX values;
@@ -342,58 +344,65 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         }
         __syncthreads();
 
-        // =============== X2: x-analysis of this CTA's column units; delete modes, prefactor, add ===============
-#pragma unroll 1
-        for (int unit = rank; unit < K::NUNIT; unit += G) {
+        // =============== X2: x-analysis of this CTA's column units (all UPC of them at once); delete modes, prefactor, add ===============
+        {
+            constexpr int UPC = K::UPC;
             // rhs values of this thread's share of stage 2, requested ahead of stage 1
             cplx r0[AX1], r1[AX1];
-            const int k2s = tid % BX, cols = (tid / BX) % CK;
-            if (tid < CK * BX) {
-                const cplx* Rcol = Rb + (size_t)(unit * CK + cols) * NX0 + k2s;
+            const int k2s = tid % BX, cols = (tid / BX) % CK, us = tid / (BX * CK);   // stage 2 item: (unit us, column, k2)
+            static_assert(UPC * CK * BX <= NT || UPC * CK * BX % NT == 0, "stage-2 items over the threads");
+#pragma unroll 1
+            for (int ub = 0; ub < UPC; ub += NT / (CK * BX)) {   // NT / (CK BX) units per pass of stage 2
+#pragma unroll 1
+                for (int i1 = tid; i1 < (NT / (CK * BX)) * CK * AX; i1 += NT) {
+                    // stage 1: unpack the row pair, radix-BX over n2 for fixed n1 (m = n1 + AX n2), twiddle
+                    const int col = i1 % CK, n1 = (i1 / CK) % AX, ul = i1 / (CK * AX);
+                    const int unit = rank + G * (ub + ul);
+                    const int kyi = unit * CK + col;
+                    const int ccm = kyi ? W2 - kyi : 0;
+                    cplx x[BX];
 #pragma unroll
-                for (int c = 0; c < AX1; ++c) {
-                    r0[c] = ldg_early(Rcol + BX * c);
-                    r1[c] = ldg_early(Rcol + BX * c + M);
+                    for (int i = 0; i < C2; ++i) {
+                        const cplx* Pr = Ps + (size_t)(n1 + AX * i) * W2;
+                        const cplx pp = ldg_cg(Pr + kyi), pm = ldg_cg(Pr + ccm);
+                        x[i] = cmake(pp.x + pm.x, pp.y - pm.y);          // 2 N^_m  = P+ + conj P-
+                        x[i + C2] = cmake(pp.y + pm.y, pm.x - pp.x);     // 2 N^_m' = -i (P+ - conj P-)
+                    }
+                    Dft<BX, -1>::run(x);
+                    cplx* Ec = A + (ul * CK + col) * CSF + n1 * BPX;
+#pragma unroll
+                    for (int k2 = 0; k2 < BX; ++k2) {
+                        const cplx w = twx[n1 * BPX + k2];
+                        Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], w.x, -w.y);
+                    }
                 }
+                const int unit2 = rank + G * (ub + us);
+                {
+                    const cplx* Rcol = Rb + (size_t)(unit2 * CK + cols) * NX0 + k2s;
+#pragma unroll
+                    for (int c = 0; c < AX1; ++c) {
+                        r0[c] = ldg_early(Rcol + BX * c);
+                        r1[c] = ldg_early(Rcol + BX * c + M);
+                    }
+                }
+                __syncthreads();
+                {  // stage 2: pruned-output radix-AX over n1 for fixed k2; i = k2 + BX c
+                    cplx in[AX];
+                    const cplx* Ec = A + (us * CK + cols) * CSF + k2s;
+#pragma unroll
+                    for (int n1 = 0; n1 < AX; ++n1) in[n1] = Ec[n1 * BPX];
+                    cplx lo[AX1], hi[AX1];
+                    dft_pruned_out<AX, -1>(in, lo, hi);
+                    cplx* Rcol = Rb + (size_t)(unit2 * CK + cols) * NX0 + k2s;
+#pragma unroll
+                    for (int c = 0; c < AX1; ++c) {
+                        Rcol[BX * c] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));
+                        if (c != 0 || k2s != 0)  // i = M is the Nyquist row: untouched (R6)
+                            Rcol[BX * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
+                    }
+                }
+                __syncthreads();  // the tiles are consumed before the next pass / the next plane's E overwrites them
             }
-            if (tid < CK * AX) {  // stage 1: unpack the row pair, radix-BX over n2 for fixed n1 (m = n1 + AX n2), twiddle
-                const int col = tid % CK, n1 = tid / CK;
-                const int kyi = unit * CK + col;
-                const int ccm = kyi ? W2 - kyi : 0;
-                cplx x[BX];
-#pragma unroll
-                for (int i = 0; i < C2; ++i) {
-                    const cplx* Pr = Ps + (size_t)(n1 + AX * i) * W2;
-                    const cplx pp = ldg_cg(Pr + kyi), pm = ldg_cg(Pr + ccm);
-                    x[i] = cmake(pp.x + pm.x, pp.y - pm.y);          // 2 N^_m  = P+ + conj P-
-                    x[i + C2] = cmake(pp.y + pm.y, pm.x - pp.x);     // 2 N^_m' = -i (P+ - conj P-)
-                }
-                Dft<BX, -1>::run(x);
-                cplx* Ec = A + col * CSF + n1 * BPX;
-#pragma unroll
-                for (int k2 = 0; k2 < BX; ++k2) {
-                    const cplx w = twx[n1 * BPX + k2];
-                    Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], w.x, -w.y);
-                }
-            }
-            __syncthreads();
-            if (tid < CK * BX) {  // stage 2: pruned-output radix-AX over n1 for fixed k2; i = k2 + BX c
-                const int k2 = k2s, col = cols;
-                cplx in[AX];
-                const cplx* Ec = A + col * CSF + k2;
-#pragma unroll
-                for (int n1 = 0; n1 < AX; ++n1) in[n1] = Ec[n1 * BPX];
-                cplx lo[AX1], hi[AX1];
-                dft_pruned_out<AX, -1>(in, lo, hi);
-                cplx* Rcol = Rb + (size_t)(unit * CK + col) * NX0 + k2;
-#pragma unroll
-                for (int c = 0; c < AX1; ++c) {
-                    Rcol[BX * c] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));
-                    if (c != 0 || k2 != 0)  // i = M is the Nyquist row: untouched (R6)
-                        Rcol[BX * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
-                }
-            }
-            __syncthreads();  // the tile is consumed before the next unit / the next plane's E overwrites it
         }
     }
 }
