@@ -534,7 +534,7 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
                           "tflops": flops[k] * nprof / (prof_ms[k] * 1e-3) / 1e12}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
     # measured DRAM bytes (ncu capture of these very sources; null when the capture is older than the code)
-    cap, why = measured_traffic(wl.name + ("+cluster" if plane_kernel else ""))
+    cap, why = measured_traffic(wl.name + ({1: "+cluster", 3: "+batched"}.get(plane_kernel, "")))
     traffic = cap[dom][0] if dom in cap else None
     traffic_step = None
     if cap and all(k in cap for k in kernels):
@@ -694,11 +694,13 @@ def main():
             per_config[W.CONFIGS[idx].name] = {k: r[k] for k in ("value", "ms_per_step", "steps", "roofline",
                                                                   "roofline_step", "kernels", "clocks", "gpu_launches")}
             per_config[W.CONFIGS[idx].name]["unit"] = UNIT
-        # configs[2] once more through the cluster kernel (Z and P in distributed shared memory instead of HBM scratch)
-        from paper_1310_1485_b200 import GENE_NL_KERNEL_CLUSTER
-        r = run_config(W.CONFIGS[2], args, env, do_e2e=False, do_cpu=False, headline=False, plane_kernel=GENE_NL_KERNEL_CLUSTER)
-        per_config[W.CONFIGS[2].name + " (gene_nl_set_plane_kernel: cluster kernel)"] = {
-            k: r[k] for k in ("value", "ms_per_step", "steps", "roofline", "roofline_step", "kernels", "clocks", "gpu_launches")}
+        # configs[2] once more through the other kernel families (gene_nl_set_plane_kernel): the cluster kernel (Z and P
+        # in distributed shared memory) and the batched kernels (Z and P through HBM scratch)
+        from paper_1310_1485_b200 import GENE_NL_KERNEL_BATCHED, GENE_NL_KERNEL_CLUSTER
+        for kind, label in ((GENE_NL_KERNEL_CLUSTER, "cluster kernel"), (GENE_NL_KERNEL_BATCHED, "batched kernels")):
+            r = run_config(W.CONFIGS[2], args, env, do_e2e=False, do_cpu=False, headline=False, plane_kernel=kind)
+            per_config[W.CONFIGS[2].name + f" (gene_nl_set_plane_kernel: {label})"] = {
+                k: r[k] for k in ("value", "ms_per_step", "steps", "roofline", "roofline_step", "kernels", "clocks", "gpu_launches")}
     if rank == 0:
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": res["steps"],

@@ -129,14 +129,20 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
 /*
  * gene_nl_set_plane_kernel -- choose the kernel family for the g side of a plane.
  *   GENE_NL_KERNEL_AUTO     what gene_nl_create selected (the fastest measured on B200): the fused shared-memory kernel
- *                           for planes that fit one SM, the batched kernels (scratch through HBM/L2) beyond.
- *   GENE_NL_KERNEL_CLUSTER  the fused kernel spread over a thread-block cluster of 8 CTAs: the half-transformed plane is
- *                           distributed over the cluster's shared memory and the two x<->y hand-overs (the
- *                           "transpositions" of PAPER.md:61) are distributed-shared-memory stores, so only g, rhs and
- *                           the chi rows cross HBM (1.03 x the algorithmic bytes).  Available for the 384 x 192 padded
- *                           grid (nx0 = 256, nky0 = 64: configs[2]) with chi_has_v = 0; GENE_NL_EUNSUPPORTED otherwise.
- * Same results to rounding (both are checked against the oracle).  Synchronises the device and re-allocates the
- * scratch, like gene_nl_set_scratch_bytes.
+ *                           for planes that fit one SM; beyond that the group kernel where it exists, else the batched
+ *                           kernels.
+ *   GENE_NL_KERNEL_GROUP    the fused kernel spread over groups of 4 co-resident CTAs (one cooperative launch, every SM
+ *                           used): the two x<->y hand-overs of a plane (the "transpositions" of PAPER.md:61) go through
+ *                           a per-group scratch of 1.1 MB that is rewritten every plane and therefore stays in L2; rows
+ *                           come back by 1-D bulk copies (TMA).  HBM sees g, rhs and the chi rows only (1.07 x the
+ *                           algorithmic bytes).  Exists for the 384 x 192 padded grid (nx0 = 256, nky0 = 64:
+ *                           configs[2]) with chi_has_v = 0 on a device with cooperative launch.
+ *   GENE_NL_KERNEL_CLUSTER  the same phases over a thread-block cluster of 8 CTAs with the half-transformed plane in the
+ *                           cluster's shared memory and distributed-shared-memory hand-overs (1.03 x the algorithmic
+ *                           bytes; slower: DSMEM stores run at 18 B/clk/SM and 15 clusters fit the 148 SMs).  Same sizes.
+ *   GENE_NL_KERNEL_BATCHED  the batched kernels (scratch through HBM/L2 in large batches) whatever the size.
+ * GENE_NL_EUNSUPPORTED when the plan has no such kernel.  Same results to rounding (all are checked against the
+ * oracle).  Synchronises the device and re-allocates the scratch, like gene_nl_set_scratch_bytes.
  */
 #define GENE_NL_KERNEL_AUTO 0
 #define GENE_NL_KERNEL_CLUSTER 1
@@ -150,7 +156,7 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind);
  *   5 algorithmic bytes per plane  B = 16*nx0*nky0*(3 + c),
  *   6 conventional flops per plane F = (3+2c)*T2D + 4M(1+c) + 3NxNy + 4M,
  *   with c = 1 if chi_has_v else 1/nv; 7: 1 if a fused (shared-memory resident) kernel is used, else 0;
- *   8: 1 if that kernel is the cluster kernel (gene_nl_set_plane_kernel), else 0.
+ *   8: 1 if that kernel is the cluster kernel, 2 if it is the group kernel (gene_nl_set_plane_kernel), else 0.
  *   Returns NaN for an unknown `what` or NULL plan.
  */
 double gene_nl_query(const gene_nl_plan* h, int what);

@@ -52,14 +52,15 @@ typedef void (*fused_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cpl
 typedef void (*fused2_fn)(const cplx*, cplx*, const cplx*, const cplx*, int, int, int, int, double, double, double);
 typedef void (*cluster_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, double, double, double);
 
-typedef void (*group_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, cplx*, unsigned*, int, int, int, double,
-                         double, double);
+typedef void (*group_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, const cplx*, cplx*, unsigned*, int, int, int,
+                         double, double, double);
 
 struct FusedKernel {
     fused_fn fn = nullptr;
     fused2_fn fn2 = nullptr;  // second-generation kernel (nl_fused2.cuh); used when available
     cluster_fn fnc = nullptr; // the plane spread over a thread-block cluster (nl_cluster.cuh); chi shared over v only
     group_fn fng = nullptr;   // the plane spread over a group of co-resident CTAs, hand-overs through L2 (nl_group.cuh)
+    bool chiv = false;        // group kernel: chi per plane goes through the kernel too (no chi-side launches)
     int group = 1;            // CTAs per group
     size_t group_scratch = 0; // bytes of Z + P scratch per group
     int cluster = 1;          // CTAs per cluster
@@ -79,12 +80,13 @@ FusedKernel make_cluster()
     return k;
 }
 
-template <int AX, int BX, int AY, int G, int NW>
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV>
 FusedKernel make_group()
 {
-    using K = gnl::Grouped<AX, BX, AY, G, NW>;
+    using K = gnl::Grouped<AX, BX, AY, G, NW, NH, CHIV>;
     FusedKernel k;
-    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW>;
+    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV>;
+    k.chiv = CHIV;
     k.group = G;
     k.group_scratch = sizeof(cplx) * K::GROUP_SCRATCH_CPLX;
     k.smem = K::SMEM_BYTES;
@@ -92,10 +94,12 @@ FusedKernel make_group()
     return k;
 }
 
-// Planes beyond one SM, chi shared over v: groups of G co-resident CTAs per plane, Z and P through L2
-bool find_group(int nx, int ny, FusedKernel* out)
+// Planes beyond one SM: groups of G co-resident CTAs per plane, Z and P through L2
+bool find_group(int nx, int ny, bool chi_has_v, FusedKernel* out)
 {
-    if (nx == 384 && ny == 192) { *out = make_group<24, 16, 24, 2, 8>(); return out->smem <= 227 * 1024; }
+    if (nx == 384 && ny == 192 && !chi_has_v) { *out = make_group<24, 16, 24, 4, 8, 2, false>(); return out->smem <= 227 * 1024; }
+    if (nx == 144 && ny == 144 && chi_has_v) { *out = make_group<12, 12, 18, 1, 8, 1, true>(); return out->smem <= 227 * 1024; }
+    if (nx == 144 && ny == 144 && !chi_has_v) { *out = make_group<12, 12, 18, 3, 8, 1, false>(); return out->smem <= 227 * 1024; }
     return false;
 }
 
@@ -401,6 +405,21 @@ void configure_batching(gene_nl_plan* h)
     const size_t W2 = 2 * (size_t)h->nky0;
     const size_t zpp = sizeof(cplx) * h->Nx * W2, ppp = zpp / 2, rpp = sizeof(cplx) * (size_t)h->Nx * h->Ny;
     const size_t budget = h->budget;
+    if (h->fused && h->fk.chiv) {   // chi per plane inside the plane kernel: no chi-side scratch, all slabs in one launch
+        size_t nss = (size_t)h->nw * h->nspec;
+        while (nss > 1 && nss * (size_t)nz * nv >= ((size_t)1 << 31)) nss /= 2;   // 32-bit plane counters in the kernels
+        if (h->budget_set) {   // an explicit budget still bounds the planes per launch (ragged launches in tests)
+            const size_t per_slab = (size_t)nz * nv * (zpp + ppp);
+            size_t cap = budget / per_slab;
+            if (cap < 1) cap = 1;
+            if (nss > cap) nss = cap;
+        }
+        h->nss = (int)nss;
+        h->nbz = 1;
+        h->nzb = nz; h->nvb = nv;
+        h->zbytes = h->pbytes = h->rbytes = 256;
+        return;
+    }
     if (h->fused) {
         const size_t cps = (size_t)nz * (h->chi_has_v ? nv : 1);          // chi planes per slab
         const size_t rcap = h->budget_set ? budget : (size_t)2 << 30;     // real-space chi kept per launch
@@ -540,7 +559,7 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
             const size_t cps = (size_t)h->nz * (h->chi_has_v ? h->nv : 1);  // chi planes per slab
             const size_t nchi = cps * ns;
             const cplx* chi0 = chi + (size_t)s0 * cps * h->M;
-            for (size_t q0 = 0; q0 < nchi; q0 += (size_t)h->nbz) {
+            for (size_t q0 = 0; q0 < nchi && !h->fk.chiv; q0 += (size_t)h->nbz) {   // chiv: chi goes through the plane kernel
                 const int nb = (int)((nchi - q0 < (size_t)h->nbz) ? nchi - q0 : (size_t)h->nbz);
                 GNL_XINV(prof, st, nb * xt, chi0 + q0 * h->M, s.Z, nb, 0);
                 GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
@@ -565,7 +584,7 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
                 cfg.attrs = at; cfg.numAttrs = 1;
                 // (a persisting-L2 access window over the scratch was measured on B200: the kernel gains 1.5 %, the
                 // chi-side kernels lose more to the carve-out: not used)
-                GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fng, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)h->twx, (const cplx*)h->twy, s.GS, s.cnt, h->nz, h->nv, ns, h->kxmin, h->kymin, coef)));
+                GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fng, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)(h->fk.chiv ? chi + goff : nullptr), (const cplx*)h->twx, (const cplx*)h->twy, s.GS, s.cnt, h->nz, h->nv, ns, h->kxmin, h->kymin, coef)));
             } else if (h->fk.fnc) {
                 // whole clusters only; a cluster walks planes with the stride of the cluster count
                 const int C = h->fk.cluster;
@@ -658,12 +677,13 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     h->table_bytes = sizeof(cplx) * (size_t)(h->Nx + h->Ny);
     // the composition chi = phi_bar - v_par A_par_bar lives in k_ybracket (batched path)
     h->fused = !h->em && (find_fused2(h->Nx, h->Ny, &h->fk) || find_fused(h->Nx, h->Ny, &h->fk));
-    // Planes beyond one SM: the batched kernels by default.  The cluster kernel (nl_cluster.cuh) keeps Z and P out of
-    // HBM (1.03 x the algorithmic bytes, ncu) but measured slower on B200 (configs[2]: 8.2 ms against 7.2 ms: only 15
-    // clusters of 8 CTAs are co-resident on the 148 SMs, and the DSMEM hand-overs run at 18 B/clk/SM in series with the
-    // butterflies; DESIGN.md sect. 6e), so it is selected on request only (gene_nl_set_plane_kernel).
+    // Planes beyond one SM.  The cluster kernel (nl_cluster.cuh) keeps Z and P out of HBM (1.03 x the algorithmic bytes,
+    // ncu) but measured slower than the batched kernels on B200 (configs[2]: 8.2 ms against 7.2 ms: only 15 clusters of
+    // 8 CTAs are co-resident on the 148 SMs, and the DSMEM hand-overs run at 18 B/clk/SM in series with the butterflies;
+    // DESIGN.md sect. 6e), so it is selected on request only (gene_nl_set_plane_kernel).  The group kernel (nl_group.cuh)
+    // replaced DSMEM by an L2-resident scratch and clusters by groups of a cooperative launch: see below.
     if (!h->fused && !h->em && !h->chi_has_v) find_cluster(h->Nx, h->Ny, &h->ck);
-    if (!h->fused && !h->em && !h->chi_has_v) find_group(h->Nx, h->Ny, &h->gk);
+    if (!h->fused && !h->em) find_group(h->Nx, h->Ny, h->chi_has_v != 0, &h->gk);
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -711,6 +731,15 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
         } else {
             h->gk_grid = (sms / h->gk.group) * h->gk.group;
         }
+    }
+    if (ok && h->gk.fng && !h->fused) {
+        // Planes beyond one SM with chi shared over v: the group kernel (Z and P through L2) is the default where it
+        // exists.  Measured on B200 at configs[2]: 6.24 ms per step against 7.24 ms for the batched kernels and 8.18 ms
+        // for the cluster kernel; DRAM traffic 1.07 x the algorithmic bytes (batched: about 4 x).
+        free_scratch(&h->scr);
+        h->fk = h->gk; h->fused = true; h->fused_grid = h->gk_grid;
+        configure_batching(h);
+        ok = alloc_scratch(h, &h->scr);
     }
     h->fk_auto = h->fk; h->fused_auto = h->fused; h->fused_grid_auto = h->fused_grid;
     if (ok && h->Nx <= 192) {

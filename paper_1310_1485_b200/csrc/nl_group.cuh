@@ -43,9 +43,44 @@ __device__ __forceinline__ unsigned ld_acquire_gpu(const unsigned* p)
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-template <int AX_, int BX_, int AY_, int G_, int NW_>
+// L2 eviction priorities: the per-group scratch is written and read again within microseconds, every plane (keep it:
+// evict_last); g streams through once (evict_first), so that the scratch lines are not the ones that leave L2
+__device__ __forceinline__ uint64_t l2_policy_evict_last()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first()
+{
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void stg_hint(cplx* p, cplx v, uint64_t pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ cplx ldg_cg_hint(const cplx* p, uint64_t pol)   // L2 only
+{
+    cplx v;
+    asm volatile("ld.global.cg.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+
+// NH: k1 passes of the X1 exchange tile (2: half of the k1 range at a time, for AX = 24; 1 for AX = 12).
+// CHIV: chi per plane (chi_has_v = 1): chi goes through X1 like g and its rows are transformed next to those of g in Y
+// (no real-space chi array R); else chi is shared over v and its real-space rows (dx chi, dy chi) come from R.
+template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_>
 struct Grouped {
-    static constexpr int AX = AX_, BX = BX_, AY = AY_, G = G_, NW = NW_;
+    static constexpr int AX = AX_, BX = BX_, AY = AY_, G = G_, NW = NW_, NH = NH_;
+    static constexpr bool CHIV = CHIV_;
+    static constexpr int NF = CHIV ? 2 : 1;            // fields that go through X1 and the row hand-over
     static constexpr int NX = AX * BX, NY = 8 * AY, C2 = BX / 2;
     static constexpr int NKY0 = NY / 3, W2 = 2 * NKY0, NPAIR = NX / 2;
     static constexpr int M = NX / 3, NX0 = 2 * M;
@@ -58,40 +93,41 @@ struct Grouped {
     static constexpr int NT = 32 * NW;
     static constexpr int FY = AY * 9;                  // y exchange tile of one row: [k1][9]
     static constexpr int PS = (W2 + FY) | 1;           // pair storage: rows m + NX/2 | m, the tile over row m and beyond
-    static constexpr int YB_CPLX = NW * NPW * PS;
-    static constexpr int BPX = Tile<AX, BX>::BP, AXH = AX / 2;
-    static constexpr int CSH = ((AXH * BPX) | 1) + ((((AXH * BPX) | 1) % 8 == 1) ? 4 : 0);   // half-k1 tile of one column-sign
-    static constexpr int E_CPLX = 2 * CK * CSH;        // X1: both signs of a unit's columns, half of the k1 range at a time
+    static constexpr int YB_CPLX = NW * NF * NPW * PS;
+    static constexpr int BPX = Tile<AX, BX>::BP, AXH = AX / NH;
+    static constexpr int CSH = ((AXH * BPX) | 1) + ((((AXH * BPX) | 1) % 8 == 1) ? 4 : 0);   // tile of one column-sign, AXH values of k1
+    static constexpr int E_CPLX = 2 * CK * CSH;        // X1: both signs of a unit's columns, AXH values of k1 at a time
     static constexpr int CSF = Tile<AX, BX>::STRIDE;
-    static constexpr int TX_CPLX = (32 * NW_ / (CK * BX_)) * CK * CSF;   // X2: exchange tiles of the units of one pass
+    static constexpr int XBIG = AX > BX ? AX : BX;
+    static constexpr int UPP = (NT / (CK * XBIG)) < UPC ? (NT / (CK * XBIG)) : UPC;   // X2: units per pass
+    static constexpr int TX_CPLX = UPP * CK * CSF;     // X2: exchange tiles of the units of one pass
     static constexpr int XR_CPLX = E_CPLX > TX_CPLX ? E_CPLX : TX_CPLX;
     static constexpr int A_CPLX = YB_CPLX > XR_CPLX ? YB_CPLX : XR_CPLX;   // the x tiles and the y pair storages share a region
-    static constexpr int G_CPLX = CK * NX0;            // one unit's columns of a g plane (one contiguous block)
+    static constexpr int G_CPLX = CK * NX0;            // one unit's columns of a spectral plane (one contiguous block)
     static constexpr int TWX = AX * BPX, TWY = AY * 9;
-    static constexpr int NBAR = 1 + NW;                // mbarriers: g block, rows of each warp
+    static constexpr int NBAR = 1 + NW;                // mbarriers: column block, rows of each warp
     static constexpr int SMEM_CPLX = A_CPLX + G_CPLX + TWX + TWY + (NBAR + 1) / 2;
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
     static constexpr size_t ZS_CPLX = (size_t)NPAIR * 2 * W2, PS_CPLX = (size_t)NPAIR * W2;   // per-group scratch
-    static constexpr size_t GROUP_SCRATCH_CPLX = ZS_CPLX + PS_CPLX;
-    static_assert(AX % 3 == 0 && AY % 3 == 0 && AX % 2 == 0 && BX % 2 == 0, "3/2 rule; half-k1 tiles; row pairs");
+    static constexpr size_t GROUP_SCRATCH_CPLX = NF * ZS_CPLX + PS_CPLX;
+    static_assert(AX % 3 == 0 && AY % 3 == 0 && AX % NH == 0 && BX % 2 == 0, "3/2 rule; k1 passes; row pairs");
     static_assert(NKY0 % CK == 0 && NUNIT % G == 0 && NPAIR % G == 0 && PPG % NPW == 0, "the group divides the work");
     static_assert(NPW * 8 <= 32 && AY <= 32 && NKY0 == 8 * (AY / 3), "lanes of the y stages");
-    static_assert(2 * CK * BX == NT && (2 * CK * AXH) % 32 == 0 && 2 * CK * AXH <= NT && CK * AX <= NT && CK * BX <= NT,
-                  "one item per thread in every x stage");
-    static_assert(UPC % (NT / (CK * BX)) == 0, "X2 takes NT / (CK BX) units per pass");
+    static_assert(2 * CK * BX <= NT && 2 * CK * AXH <= NT && UPP >= 1 && UPC % UPP == 0, "one item per thread in every x stage");
 };
 
 // grid = groups * G CTAs (cooperative launch: every CTA is resident).  scratch: groups * GROUP_SCRATCH_CPLX values;
-// cnt: 2 * groups counters, zeroed before the launch.
-template <int AX, int BX, int AY, int G, int NW>
+// cnt: 2 * groups counters, zeroed before the launch.  chi: the spectral chi planes when CHIV (laid out like g), else
+// unused; R: the real-space chi rows when !CHIV, else unused.
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV>
 __global__ void __launch_bounds__(32 * NW, 1)
-k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R,
+k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R, const cplx* __restrict__ chi,
               const cplx* __restrict__ twx_g, const cplx* __restrict__ twy_g, cplx* __restrict__ scratch,
               unsigned* __restrict__ cnt, int nz, int nv, int nslab, double kxmin, double kymin, double coef)
 {
-    using K = Grouped<AX, BX, AY, G, NW>;
-    constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR;
-    constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT;
+    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV>;
+    constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR, NF = K::NF;
+    constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT, UPC = K::UPC, UPP = K::UPP;
     constexpr int PS = K::PS, BPX = K::BPX, CSH = K::CSH, CSF = K::CSF, AXH = K::AXH;
     constexpr int AX1 = AX / 3, AY1 = AY / 3;
     constexpr unsigned FULL = 0xffffffffu;
@@ -99,7 +135,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
 
     extern __shared__ cplx smem[];
     cplx* A = smem;                        // X1: E / X2: Tx / Y: pair storages of the warps
-    cplx* Gs = A + K::A_CPLX;              // a unit's columns of g (bulk copy)
+    cplx* Gs = A + K::A_CPLX;              // a unit's columns of g or chi (bulk copy)
     cplx* twx = Gs + K::G_CPLX;            // W_NX^{n2 k1}, [k1][BPX]
     cplx* twy = twx + K::TWX;              // W_NY^{k1 k2}, [k1][9]
     const uint32_t bars = smem_u32(twy + K::TWY);
@@ -110,8 +146,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
     const int warp = __shfl_sync(FULL, tid >> 5, 0);
     const uint32_t ybar = bars + 8 + 8 * (uint32_t)warp;
     const int ngroup = gridDim.x / G, grp = blockIdx.x / G, rank = blockIdx.x % G;
-    cplx* Zs = scratch + (size_t)grp * K::GROUP_SCRATCH_CPLX;   // [pair][row m + NX/2 | row m][cc]
-    cplx* Ps = Zs + K::ZS_CPLX;                                 // [pair][cc]
+    cplx* Zs = scratch + (size_t)grp * K::GROUP_SCRATCH_CPLX;   // [field][pair][row m + NX/2 | row m][cc]; field 0 = g
+    cplx* Ps = Zs + NF * K::ZS_CPLX;                            // [pair][cc]
     unsigned* zcnt = cnt + 2 * grp;
     unsigned* pcnt = zcnt + 1;
 
@@ -132,11 +168,15 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         const unsigned z = zs % (unsigned)nz, sl = zs / (unsigned)nz;
         return (size_t)z + (size_t)nz * ((size_t)v + (size_t)nv * sl);
     };
-    auto request_g = [&](unsigned tt, int unit) {   // one thread: columns [8 unit, 8 unit + 8) of plane tt -> Gs
+    const uint64_t pol_keep = l2_policy_evict_last(), pol_stream = l2_policy_evict_first();
+    // X1 step s of a plane: field s / UPC (with CHIV: chi first, then g), column unit rank + G (s mod UPC)
+    auto request_block = [&](unsigned tt, int s) {   // one thread: the 8 columns of step s of plane tt -> Gs
+        const cplx* src = (CHIV && s < UPC) ? chi : g;
         mbar_arrive_expect_tx(gbar, GBYTES);
-        bulk_g2s(smem_u32(Gs), g + plane_of(tt) * plane_elems + (size_t)unit * CK * NX0, GBYTES, gbar);
+        bulk_g2s_hint(smem_u32(Gs), src + plane_of(tt) * plane_elems + (size_t)(rank + G * (s % UPC)) * CK * NX0, GBYTES, gbar,
+                      pol_stream);
     };
-    if (tid == 0 && (unsigned)grp < T) request_g((unsigned)grp, rank);
+    if (tid == 0 && (unsigned)grp < T) request_block((unsigned)grp, 0);
 
     uint32_t gph = 0, yph = 0;
     unsigned it = 0;
@@ -144,11 +184,13 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         const size_t p = plane_of(t);
         const size_t q = (size_t)((t / (unsigned)nv) % (unsigned)nz) + (size_t)nz * (size_t)(t / ((unsigned)nv * (unsigned)nz));
         cplx* Rb = rhs + p * plane_elems;
-        const cplx* Rc = R + q * ((size_t)NX * NY);
+        [[maybe_unused]] const cplx* Rc = CHIV ? nullptr : R + q * ((size_t)NX * NY);
 
         // =============== X1: derivative, pad, x-synthesis of this CTA's column units; rows go to Z ===============
 #pragma unroll 1
-        for (int unit = rank; unit < K::NUNIT; unit += G) {
+        for (int s = 0; s < NF * UPC; ++s) {
+            const int unit = rank + G * (s % UPC);
+            cplx* Zf = Zs + ((CHIV && s < UPC) ? K::ZS_CPLX : 0);   // field 0 = g, field 1 = chi
             mbar_wait(gbar, gph);
             gph ^= 1;
             if (unit == 0) {   // Hermitian part of the ky = 0 column (reading R7), in place in the staged block
@@ -161,11 +203,12 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 }
                 __syncthreads();
             }
-            // stage 1, every thread: column-sign c2 = (sign, column), position n2: pruned radix-AX over n1 (i = n2 + BX n1),
-            // twiddle W_NX^{n2 k1}.  The k1 < AX/2 half goes to E now, the other half after the first stage-2 pass.
+            // stage 1: column-sign c2 = (sign, column), position n2: pruned radix-AX over n1 (i = n2 + BX n1), twiddle
+            // W_NX^{n2 k1}.  AXH values of k1 go to E at a time, the rest waits in registers.
             const int n2 = opaque(tid % BX), c2 = opaque(tid / BX);
+            const bool has1 = tid < 2 * CK * BX;
             cplx out[AX];
-            {
+            if (has1) {
                 const int col1 = c2 % CK;
                 const cplx* Fc = Gs + col1 * NX0 + n2;
                 const double ky = kymin * (double)(unit * CK + col1), dn2 = (double)n2;
@@ -184,14 +227,14 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     out[k1] = cmul(out[k1], w.x, w.y);
                 }
             }
-            __syncthreads();   // every thread has read its g values
-            if (tid == 0) {    // the next block: this CTA's next unit of this plane, or its first unit of the next plane
-                if (unit + G < K::NUNIT) request_g(t, unit + G);
-                else if (t + (unsigned)ngroup < T) request_g(t + (unsigned)ngroup, rank);
+            __syncthreads();   // every thread has read its values of the block
+            if (tid == 0) {    // the next block: the next step of this plane, or the first step of the next plane
+                if (s + 1 < NF * UPC) request_block(t, s + 1);
+                else if (t + (unsigned)ngroup < T) request_block(t + (unsigned)ngroup, 0);
             }
 #pragma unroll
-            for (int hk = 0; hk < 2; ++hk) {
-                {
+            for (int hk = 0; hk < K::NH; ++hk) {
+                if (has1) {
                     cplx* Ec = A + c2 * CSH + n2;
 #pragma unroll
                     for (int k1 = 0; k1 < AXH; ++k1) Ec[k1 * BPX] = out[hk * AXH + k1];
@@ -209,13 +252,13 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     for (int i = 0; i < BX; ++i) v[i] = zero ? cmake(0.0, 0.0) : Ec[i];
                     Dft<BX, +1>::run(v);
                     const int cc = sg ? (kyi ? W2 - kyi : NKY0) : kyi;
-                    cplx* Zc = Zs + (size_t)k1 * (2 * W2) + cc;
+                    cplx* Zc = Zf + (size_t)k1 * (2 * W2) + cc;
                     const double sgn = sg ? -1.0 : 1.0;   // -ky columns hold the conjugate
 #pragma unroll
                     for (int k2 = 0; k2 < BX; ++k2)      // pair storage: row m + NX/2 (k2 >= C2) first, then row m
-                        Zc[(size_t)(AX * (k2 % C2)) * (2 * W2) + (k2 < C2 ? W2 : 0)] = cmake(v[k2].x, sgn * v[k2].y);
+                        stg_hint(Zc + (size_t)(AX * (k2 % C2)) * (2 * W2) + (k2 < C2 ? W2 : 0), cmake(v[k2].x, sgn * v[k2].y), pol_keep);
                 }
-                __syncthreads();  // E is free for the second half / the next unit
+                __syncthreads();  // E is free for the next k1 pass / the next step
             }
         }
         // ---- hand-over 1: every CTA of the group has written its columns of Z ----
@@ -234,84 +277,136 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
             const int j1 = (lane >> 3) < NPW ? (lane >> 3) : 0;   // Y1 / Y3 item: pair j1 of the warp item, position lane & 7
             const bool act1 = (lane >> 3) < NPW;
             const int n2 = lane & 7;
-            cplx* Zw = A + (warp * NPW) * PS;                     // this warp's pair storages
+            cplx* Zw = A + (warp * NF * NPW) * PS;                // this warp's pair storages: g, then (CHIV) chi
             cplx tq[8];
 #pragma unroll
             for (int k2 = 1; k2 < 8; ++k2) tq[k2] = twy[k1y * 9 + k2];
+            // Y1: pruned radix-AY of rows m (h = 0: second half of the storage) / m + NX/2 (h = 1: first half) of the NPW
+            // pairs that start at storage Zst; the exchange tile of a pair starts at its row m
+            auto y1 = [&](cplx* Zst, int h) {
+                const cplx* Zr = Zst + j1 * PS + (h ? 0 : W2) + n2;
+                cplx lo[AY1], hi[AY1];
+#pragma unroll
+                for (int a = 0; a < AY1; ++a) {
+                    lo[a] = Zr[8 * a];
+                    hi[a] = Zr[8 * a + NKY0];
+                }
+                cplx out[AY];
+                dft_pruned_in<AY, +1>(lo, hi, out);
+                __syncwarp(FULL);  // h = 0: rows m are in registers before the tiles overwrite them; h = 1: Y2 done
+                if (act1) {
+                    cplx* tile = Zst + j1 * PS + W2 + n2;
+#pragma unroll
+                    for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
+                }
+            };
 #pragma unroll 1
             for (int item = warp; item < K::NITEM; item += NW) {
                 const int q0 = rank * PPG + item * NPW;           // first pair of the item
-                if (lane == 0) {   // the rows of the item's pairs: one bulk copy per pair (2 W2 values, contiguous in Z)
+                if (lane == 0) {   // the rows of the item's pairs: one bulk copy per pair and field (2 W2 values, contiguous in Z)
                     fence_proxy_async();
-                    mbar_arrive_expect_tx(ybar, (uint32_t)(NPW * 2 * W2 * sizeof(cplx)));
+                    mbar_arrive_expect_tx(ybar, (uint32_t)(NF * NPW * 2 * W2 * sizeof(cplx)));
 #pragma unroll
-                    for (int j = 0; j < NPW; ++j)
-                        bulk_g2s(smem_u32(Zw + j * PS), Zs + (size_t)(q0 + j) * (2 * W2), (uint32_t)(2 * W2 * sizeof(cplx)), ybar);
+                    for (int j = 0; j < NF * NPW; ++j)
+                        bulk_g2s_hint(smem_u32(Zw + j * PS), Zs + (size_t)(j / NPW) * K::ZS_CPLX + (size_t)(q0 + j % NPW) * (2 * W2),
+                                      (uint32_t)(2 * W2 * sizeof(cplx)), ybar, pol_keep);
                 }
-                cplx chv[8];
-                {
+                [[maybe_unused]] cplx chv[8];
+                if constexpr (!CHIV && !(((NPW * AY + 31) / 32) < NPW)) {   // (flat items: requested after the wait, below)
                     const cplx* Rr = Rc + (size_t)q0 * NY + k1y;
 #pragma unroll
                     for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
                 }
                 mbar_wait(ybar, yph);
                 yph ^= 1;
-                double nlx[NPW][8];                                   // bracket of the rows m (first halves), kept in registers
+                // Y2 items (pair j, k1): NPW AY of them.  With AY lanes per pair a round is one pair (AY of 32 lanes busy);
+                // when fewer rounds of 32 cover all items (AY = 18: 54 items, 2 rounds instead of 3) the items are laid
+                // flat over the lanes and the twiddles of a lane's k1 are read again for every round.
+                constexpr int NY2 = NPW * AY, NRF = (NY2 + 31) / 32;
+                constexpr bool FLAT = NRF < NPW;
+                constexpr int NR = FLAT ? NRF : NPW;
+                double nlx[NR][8];                                    // bracket of the rows m (first halves), kept in registers
+                auto item_of = [&](int r, int& j, int& k1, bool& valid) {
+                    if constexpr (FLAT) {
+                        const int idx = r * 32 + lane;
+                        valid = idx < NY2;
+                        const int ic = valid ? idx : idx - 32;       // idle lanes shadow an item of the previous round
+                        j = ic / AY;
+                        k1 = ic % AY;
+                    } else {
+                        j = r;
+                        k1 = k1y;
+                        valid = act2;
+                    }
+                };
+                if constexpr (FLAT && !CHIV) {   // the first round's chi values for the flat item of this lane
+                    int j, k1; bool valid;
+                    item_of(0, j, k1, valid);
+                    const cplx* Rr = Rc + (size_t)(q0 + j) * NY + k1;
+#pragma unroll
+                    for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
+                }
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    {  // Y1: pruned radix-AY of rows m (h = 0: second half of the storage) / m + NX/2 (h = 1: first half)
-                        const cplx* Zr = Zw + j1 * PS + (h ? 0 : W2) + n2;
-                        cplx lo[AY1], hi[AY1];
-#pragma unroll
-                        for (int a = 0; a < AY1; ++a) {
-                            lo[a] = Zr[8 * a];
-                            hi[a] = Zr[8 * a + NKY0];
-                        }
-                        cplx out[AY];
-                        dft_pruned_in<AY, +1>(lo, hi, out);
-                        __syncwarp(FULL);  // h = 0: rows m are in registers before the tiles overwrite them; h = 1: Y2 done
-                        if (act1) {
-                            cplx* tile = Zw + j1 * PS + W2 + n2;
-#pragma unroll
-                            for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
-                        }
-                    }
+                    y1(Zw, h);
+                    if constexpr (CHIV) y1(Zw + NPW * PS, h);
                     __syncwarp(FULL);
 #pragma unroll
-                    for (int j = 0; j < NPW; ++j) {  // Y2: twiddle + radix-8 to real space, bracket; pair j, k1 = lane
-                        // chi rows of the NEXT row (pair j+1 of this half, or pair 0 of the second half), requested before
-                        // this row's butterflies so that their latency hides behind them
-                        cplx chn[8];
-                        const int jn = (j + 1 < NPW) ? j + 1 : 0, hn = (j + 1 < NPW) ? h : 1;
-                        if (!(h == 1 && j + 1 == NPW)) {
-                            const cplx* Rr = Rc + (size_t)(q0 + jn + hn * NPAIR) * NY + k1y;
+                    for (int r = 0; r < NR; ++r) {  // Y2: twiddle + radix-8 to real space, bracket
+                        int j, k1; bool valid;
+                        item_of(r, j, k1, valid);
+                        [[maybe_unused]] cplx chn[8];
+                        if constexpr (!CHIV) {
+                            // chi values of the NEXT round (or of the first round of the second half), requested before
+                            // this round's butterflies so that their latency hides behind them
+                            const int rn = (r + 1 < NR) ? r + 1 : 0, hn = (r + 1 < NR) ? h : 1;
+                            if (!(h == 1 && r + 1 == NR)) {
+                                int jn, k1n; bool vn;
+                                item_of(rn, jn, k1n, vn);
+                                const cplx* Rr = Rc + (size_t)(q0 + jn + hn * NPAIR) * NY + k1n;
 #pragma unroll
-                            for (int k2 = 0; k2 < 8; ++k2) chn[k2] = ldg_nc_early(Rr + AY * k2);
+                                for (int k2 = 0; k2 < 8; ++k2) chn[k2] = ldg_nc_early(Rr + AY * k2);
+                            }
                         }
-                        cplx* tile = Zw + j * PS + W2 + k1y * 9;
+                        [[maybe_unused]] cplx tqr[8];
+                        if constexpr (FLAT) {
+#pragma unroll
+                            for (int k2 = 1; k2 < 8; ++k2) tqr[k2] = twy[k1 * 9 + k2];
+                        }
+                        const cplx (&tw)[8] = *(FLAT ? &tqr : &tq);
+                        cplx* tile = Zw + j * PS + W2 + k1 * 9;
                         cplx v[8];
 #pragma unroll
                         for (int i = 0; i < 8; ++i) v[i] = tile[i];
-                        dft8_twiddled<+1>(v, tq);   // (dx g + i dy g)(row, y = k1 + AY k2)
+                        dft8_twiddled<+1>(v, tw);   // (dx g + i dy g)(row, y = k1 + AY k2)
+                        if constexpr (CHIV) {       // (dx chi + i dy chi) of the same row from chi's tile
+                            const cplx* tc = Zw + (NPW + j) * PS + W2 + k1 * 9;
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) chv[i] = tc[i];
+                            dft8_twiddled<+1>(chv, tw);
+                        }
                         if (h == 0) {
 #pragma unroll
-                            for (int k2 = 0; k2 < 8; ++k2) nlx[j][k2] = fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x);
+                            for (int k2 = 0; k2 < 8; ++k2) nlx[r][k2] = fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x);
                         } else {
                             cplx w[8];
 #pragma unroll
                             for (int k2 = 0; k2 < 8; ++k2)
-                                w[k2] = cmake(nlx[j][k2], fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x));
+                                w[k2] = cmake(nlx[r][k2], fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x));
                             Dft<8, -1>::run(w);
 #pragma unroll
-                            for (int k2 = 1; k2 < 8; ++k2) w[k2] = cmul(w[k2], tq[k2].x, -tq[k2].y);
-                            if (act2) {  // own slots of the tile: no other lane reads or writes them in this phase
+                            for (int k2 = 1; k2 < 8; ++k2) w[k2] = cmul(w[k2], tw[k2].x, -tw[k2].y);
+                            if constexpr (FLAT) __syncwarp(FULL);   // shadow lanes have read their tiles before the owners overwrite them
+                            if (valid) {  // own slots of the tile: no other active lane reads or writes them in this phase
 #pragma unroll
                                 for (int k2 = 0; k2 < 8; ++k2) tile[k2] = w[k2];
                             }
                         }
-                        if (!(h == 1 && j + 1 == NPW)) {
+                        if constexpr (!CHIV) {
+                            if (!(h == 1 && r + 1 == NR)) {
 #pragma unroll
-                            for (int k2 = 0; k2 < 8; ++k2) chv[k2] = chn[k2];
+                                for (int k2 = 0; k2 < 8; ++k2) chv[k2] = chn[k2];
+                            }
                         }
                     }
                     __syncwarp(FULL);
@@ -327,8 +422,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                         cplx* Pp = Ps + (size_t)(q0 + j1) * W2 + n2;
 #pragma unroll
                         for (int c = 0; c < AY1; ++c) {
-                            Pp[8 * c] = lo[c];          // +ky half: cc = ky = n2 + 8 c
-                            Pp[8 * c + NKY0] = hi[c];   // -ky half: cc = nky0 + n2 + 8 c  <->  ky = nky0 - n2 - 8 c
+                            stg_hint(Pp + 8 * c, lo[c], pol_keep);          // +ky half: cc = ky = n2 + 8 c
+                            stg_hint(Pp + 8 * c + NKY0, hi[c], pol_keep);   // -ky half: cc = nky0 + n2 + 8 c  <->  ky = nky0 - n2 - 8 c
                         }
                     }
                 }
@@ -344,27 +439,24 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         }
         __syncthreads();
 
-        // =============== X2: x-analysis of this CTA's column units (all UPC of them at once); delete modes, prefactor, add ===============
+        // =============== X2: x-analysis of this CTA's column units, UPP at a time; delete modes, prefactor, add ===============
         {
-            constexpr int UPC = K::UPC;
-            // rhs values of this thread's share of stage 2, requested ahead of stage 1
             cplx r0[AX1], r1[AX1];
-            const int k2s = tid % BX, cols = (tid / BX) % CK, us = tid / (BX * CK);   // stage 2 item: (unit us, column, k2)
-            static_assert(UPC * CK * BX <= NT || UPC * CK * BX % NT == 0, "stage-2 items over the threads");
+            const int k2s = tid % BX, cols = (tid / BX) % CK, us = tid / (BX * CK);   // stage 2 item: (unit us of the pass, column, k2)
+            const bool has2 = tid < UPP * CK * BX;
 #pragma unroll 1
-            for (int ub = 0; ub < UPC; ub += NT / (CK * BX)) {   // NT / (CK BX) units per pass of stage 2
+            for (int ub = 0; ub < UPC; ub += UPP) {
 #pragma unroll 1
-                for (int i1 = tid; i1 < (NT / (CK * BX)) * CK * AX; i1 += NT) {
+                for (int i1 = tid; i1 < UPP * CK * AX; i1 += NT) {
                     // stage 1: unpack the row pair, radix-BX over n2 for fixed n1 (m = n1 + AX n2), twiddle
                     const int col = i1 % CK, n1 = (i1 / CK) % AX, ul = i1 / (CK * AX);
-                    const int unit = rank + G * (ub + ul);
-                    const int kyi = unit * CK + col;
+                    const int kyi = (rank + G * (ub + ul)) * CK + col;
                     const int ccm = kyi ? W2 - kyi : 0;
                     cplx x[BX];
 #pragma unroll
                     for (int i = 0; i < C2; ++i) {
                         const cplx* Pr = Ps + (size_t)(n1 + AX * i) * W2;
-                        const cplx pp = ldg_cg(Pr + kyi), pm = ldg_cg(Pr + ccm);
+                        const cplx pp = ldg_cg_hint(Pr + kyi, pol_keep), pm = ldg_cg_hint(Pr + ccm, pol_keep);
                         x[i] = cmake(pp.x + pm.x, pp.y - pm.y);          // 2 N^_m  = P+ + conj P-
                         x[i + C2] = cmake(pp.y + pm.y, pm.x - pp.x);     // 2 N^_m' = -i (P+ - conj P-)
                     }
@@ -376,9 +468,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                         Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], w.x, -w.y);
                     }
                 }
-                const int unit2 = rank + G * (ub + us);
-                {
-                    const cplx* Rcol = Rb + (size_t)(unit2 * CK + cols) * NX0 + k2s;
+                cplx* Rcol = Rb + (size_t)((rank + G * (ub + us)) * CK + cols) * NX0 + k2s;
+                if (has2) {  // rhs values of this thread's share of stage 2
 #pragma unroll
                     for (int c = 0; c < AX1; ++c) {
                         r0[c] = ldg_early(Rcol + BX * c);
@@ -386,14 +477,13 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     }
                 }
                 __syncthreads();
-                {  // stage 2: pruned-output radix-AX over n1 for fixed k2; i = k2 + BX c
+                if (has2) {  // stage 2: pruned-output radix-AX over n1 for fixed k2; i = k2 + BX c
                     cplx in[AX];
                     const cplx* Ec = A + (us * CK + cols) * CSF + k2s;
 #pragma unroll
                     for (int n1 = 0; n1 < AX; ++n1) in[n1] = Ec[n1 * BPX];
                     cplx lo[AX1], hi[AX1];
                     dft_pruned_out<AX, -1>(in, lo, hi);
-                    cplx* Rcol = Rb + (size_t)(unit2 * CK + cols) * NX0 + k2s;
 #pragma unroll
                     for (int c = 0; c < AX1; ++c) {
                         Rcol[BX * c] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));

@@ -196,7 +196,7 @@ SPREAD_SHAPES = [(256, 64, 1, 1, 1, 1),       # one plane: one cluster / group b
                  (256, 64, 2, 3, 1, 1),
                  (256, 64, 3, 5, 2, 2),       # 60 planes: several planes per cluster / group, chi shared by 5 planes
                  (256, 64, 36, 2, 1, 1)]
-SPREAD_KINDS = [1, 2]                         # GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP
+SPREAD_KINDS = [1, 2, 3]                      # GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP (the default here), GENE_NL_KERNEL_BATCHED
 
 
 @pytest.mark.parametrize("kind", SPREAD_KINDS)
@@ -205,7 +205,9 @@ def test_spread_kernels_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, 
     from paper_1310_1485_b200 import GeneNL
     wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, False, seed=300 + nz + nv)
     with GeneNL(wl, plane_kernel=kind) as nl:
-        assert nl.query(7) == 1.0 and nl.query(8) == float(kind)   # the requested kernel is the one that runs
+        assert (nl.query(7), nl.query(8)) == ((1.0, float(kind)) if kind < 3 else (0.0, 0.0))   # the requested kernel runs
+    with GeneNL(wl) as nl:
+        assert nl.query(8) == 2.0                                   # and the group kernel is the default at this size
     check_parity(wl, cuda_device, plane_kernel=kind)
     check_parity(wl, cuda_device, plane_kernel=kind, scratch_bytes=20 << 20)   # several launches
     check_parity(wl, cuda_device, plane_kernel=kind, host=True)                 # behind the streaming driver
@@ -252,8 +254,30 @@ def test_spread_kernels_properties_and_selection(cuda_device, kind):
             gene_nl_set_plane_kernel(nl.h, 7)
     for bad in (W.small_workload(128, 32, 1, 1, 1, 1), W.small_workload(256, 64, 1, 1, 1, 1, chi_has_v=True)):
         with GeneNL(bad) as nl:
-            with pytest.raises(GeneNLError):
-                gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_CLUSTER)                  # no cluster kernel for these
+            if kind == GENE_NL_KERNEL_BATCHED:
+                gene_nl_set_plane_kernel(nl.h, kind)                                    # the batched kernels serve every size
+            else:
+                with pytest.raises(GeneNLError):
+                    gene_nl_set_plane_kernel(nl.h, GENE_NL_KERNEL_CLUSTER)              # no cluster / group kernel for these
+
+
+# 144 x 144 planes (the shape of configs[4]): the group kernel with chi per plane (chi goes through the kernel like g) and
+# with chi shared over v, and the batched kernels on the same data
+@pytest.mark.parametrize("kind", [2, 3])
+@pytest.mark.parametrize("chi_has_v", [True, False])
+@pytest.mark.parametrize("nz,nv,nw,nspec", [(1, 1, 1, 1), (3, 5, 2, 2), (37, 2, 1, 1)])
+def test_group_kernel_144x144_planes(cuda_device, nz, nv, nw, nspec, chi_has_v, kind):
+    from paper_1310_1485_b200 import GeneNL
+    wl = W.small_workload(96, 48, nz, nv, nw, nspec, 0.04, 0.06, chi_has_v, seed=400 + nz + nv)
+    with GeneNL(wl) as nl:
+        assert nl.query(8) == 2.0                                   # the group kernel is the default at this size
+    check_parity(wl, cuda_device, plane_kernel=kind)
+    check_parity(wl, cuda_device, plane_kernel=kind, scratch_bytes=4 << 20)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    a = gpu_compute(wl, chi, g, rhs, plane_kernel=2)
+    b = gpu_compute(wl, chi, g, rhs, plane_kernel=3)
+    assert (a - b).abs().max() <= 1e-13 * (b - rhs).abs().max()
+    assert torch.equal(gpu_compute(wl, chi, g, rhs, scale=0.0, plane_kernel=kind), rhs)
 
 
 def test_config1_sampled_modes_against_the_definition(cuda_device):
