@@ -372,7 +372,8 @@ def em_main(args):
     F, B = gene_nl_query(h, 6), gene_nl_query(h, 5)
     fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
     tf = F * wl.planes / (ms_per_step * 1e-3) / 1e12
-    roofline = {"kernel": "whole step (k_xinv, k_ybracket<EM>, k_xfwd; chi side 4 launches per chunk)", "bound": "alu",
+    kind = {0.0: "batched kernels (k_xinv, k_ybracket<EM>, k_xfwd)", 2.0: "group kernel k_plane_group<EM>"}.get(gene_nl_query(h, 8), "?")
+    roofline = {"kernel": f"whole step: {kind}; chi side: k_xinv + k_yreal on phi_bar and A_par_bar", "bound": "alu",
                 "achieved": tf, "peak": fp64_model, "unit": "TFLOP/s", "frac": tf / fp64_model, "traffic": None,
                 "peak_source": "model 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md sect. 7)",
                 "flops_per_plane": F, "bytes_per_plane": B}

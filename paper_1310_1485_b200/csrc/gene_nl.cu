@@ -53,7 +53,7 @@ typedef void (*fused2_fn)(const cplx*, cplx*, const cplx*, const cplx*, int, int
 typedef void (*cluster_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, int, int, int, double, double, double);
 
 typedef void (*group_fn)(const cplx*, cplx*, const cplx*, const cplx*, const cplx*, const cplx*, cplx*, unsigned*, int, int, int,
-                         double, double, double);
+                         double, double, double, const cplx*, const double*, int, int);
 
 struct FusedKernel {
     fused_fn fn = nullptr;
@@ -80,12 +80,12 @@ FusedKernel make_cluster()
     return k;
 }
 
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV>
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false>
 FusedKernel make_group()
 {
     using K = gnl::Grouped<AX, BX, AY, G, NW, NH, CHIV>;
     FusedKernel k;
-    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV>;
+    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV, EM>;
     k.chiv = CHIV;
     k.group = G;
     k.group_scratch = sizeof(cplx) * K::GROUP_SCRATCH_CPLX;
@@ -95,11 +95,16 @@ FusedKernel make_group()
 }
 
 // Planes beyond one SM: groups of G co-resident CTAs per plane, Z and P through L2
-bool find_group(int nx, int ny, bool chi_has_v, FusedKernel* out)
+bool find_group(int nx, int ny, bool chi_has_v, bool em, FusedKernel* out)
 {
+    if (em) {  // chi composed on the device from phi_bar and A_par_bar
+        if (nx == 384 && ny == 192) { *out = make_group<24, 16, 24, 4, 8, 2, false, true>(); return out->smem <= 227 * 1024; }
+        if (nx == 144 && ny == 144) { *out = make_group<12, 12, 18, 1, 8, 1, false, true>(); return out->smem <= 227 * 1024; }
+        return false;
+    }
     if (nx == 384 && ny == 192 && !chi_has_v) { *out = make_group<24, 16, 24, 4, 8, 2, false>(); return out->smem <= 227 * 1024; }
     if (nx == 144 && ny == 144 && chi_has_v) { *out = make_group<12, 12, 18, 1, 8, 1, true>(); return out->smem <= 227 * 1024; }
-    if (nx == 144 && ny == 144 && !chi_has_v) { *out = make_group<12, 12, 18, 3, 8, 1, false>(); return out->smem <= 227 * 1024; }
+    if (nx == 144 && ny == 144 && !chi_has_v) { *out = make_group<12, 12, 18, 1, 8, 1, false>(); return out->smem <= 227 * 1024; }
     return false;
 }
 
@@ -423,7 +428,7 @@ void configure_batching(gene_nl_plan* h)
     if (h->fused) {
         const size_t cps = (size_t)nz * (h->chi_has_v ? nv : 1);          // chi planes per slab
         const size_t rcap = h->budget_set ? budget : (size_t)2 << 30;     // real-space chi kept per launch
-        size_t nss = rcap / (cps * rpp);
+        size_t nss = rcap / (cps * rpp * (h->em ? 2 : 1));
         if (nss < 1) nss = 1;
         if (nss > (size_t)h->nw * h->nspec) nss = (size_t)h->nw * h->nspec;
         while (nss > 1 && nss * (size_t)nz * nv >= ((size_t)1 << 31)) nss /= 2;   // 32-bit plane counters in the kernels
@@ -436,7 +441,7 @@ void configure_batching(gene_nl_plan* h)
         h->nzb = nz; h->nvb = nv;
         h->zbytes = zpp * nbz;
         h->pbytes = 256;
-        h->rbytes = rpp * cps * nss;
+        h->rbytes = rpp * cps * nss * (h->em ? 2 : 1);   // em: phi_bar's fields, then A_par_bar's
         return;
     }
     int nzb = nz;
@@ -564,6 +569,12 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
                 GNL_XINV(prof, st, nb * xt, chi0 + q0 * h->M, s.Z, nb, 0);
                 GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
                 launches += 2;
+                if (apar) {  // em: the same two kernels on A_par_bar; its real-space fields fill the second half of R
+                    cplx* R2 = s.R + h->rbytes / (2 * sizeof(cplx));
+                    GNL_XINV(prof, st, nb * xt, apar + (size_t)s0 * cps * h->M + q0 * h->M, s.Z, nb, 0);
+                    GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, R2 + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
+                    launches += 2;
+                }
             }
             const size_t goff = (size_t)s0 * h->nz * h->nv * h->M;
             long long T = (long long)ns * h->nz * h->nv;
@@ -584,7 +595,8 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
                 cfg.attrs = at; cfg.numAttrs = 1;
                 // (a persisting-L2 access window over the scratch was measured on B200: the kernel gains 1.5 %, the
                 // chi-side kernels lose more to the carve-out: not used)
-                GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fng, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)(h->fk.chiv ? chi + goff : nullptr), (const cplx*)h->twx, (const cplx*)h->twy, s.GS, s.cnt, h->nz, h->nv, ns, h->kxmin, h->kymin, coef)));
+                GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fng, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)(h->fk.chiv ? chi + goff : nullptr), (const cplx*)h->twx, (const cplx*)h->twy, s.GS, s.cnt, h->nz, h->nv, ns, h->kxmin, h->kymin, coef,
+                                                              (const cplx*)(apar ? s.R + h->rbytes / (2 * sizeof(cplx)) : nullptr), (const double*)(apar ? h->vp_dev : nullptr), h->nw, slab0 + s0)));
             } else if (h->fk.fnc) {
                 // whole clusters only; a cluster walks planes with the stride of the cluster count
                 const int C = h->fk.cluster;
@@ -683,7 +695,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     // DESIGN.md sect. 6e), so it is selected on request only (gene_nl_set_plane_kernel).  The group kernel (nl_group.cuh)
     // replaced DSMEM by an L2-resident scratch and clusters by groups of a cooperative launch: see below.
     if (!h->fused && !h->em && !h->chi_has_v) find_cluster(h->Nx, h->Ny, &h->ck);
-    if (!h->fused && !h->em) find_group(h->Nx, h->Ny, h->chi_has_v != 0, &h->gk);
+    if (!h->fused) find_group(h->Nx, h->Ny, h->chi_has_v != 0, h->em, &h->gk);
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -853,7 +865,6 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
         set_err("gene_nl_set_plane_kernel: no group kernel for this plan (384 x 192 padded grid, chi shared over v, cooperative launch)");
         return GENE_NL_EUNSUPPORTED;
     }
-    if (kind == GENE_NL_KERNEL_BATCHED && h->em) kind = GENE_NL_KERNEL_AUTO;
     if (kind == GENE_NL_KERNEL_CLUSTER && !h->ck.fnc) {
         set_err("gene_nl_set_plane_kernel: no cluster kernel for this plan (384 x 192 padded grid, chi shared over v, a device that keeps clusters of 8 CTAs resident)");
         return GENE_NL_EUNSUPPORTED;
@@ -986,7 +997,7 @@ static int host_impl(gene_nl_plan* h, const void* chi_, const void* apar_, const
         const int nstage = 3;
         std::vector<HostStage> st(nstage);
         size_t rbytes1 = h->rbytes;  // a stage's scratch set serves one slab
-        if (h->fused) rbytes1 = sizeof(cplx) * (size_t)h->Nx * h->Ny * (size_t)h->nz * (h->chi_has_v ? h->nv : 1);
+        if (h->fused && !h->em) rbytes1 = sizeof(cplx) * (size_t)h->Nx * h->Ny * (size_t)h->nz * (h->chi_has_v ? h->nv : 1);
         bool ok = true;
         for (auto& s : st) {
             ok = ok && cuda_ok(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate") &&
@@ -1069,7 +1080,7 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h)
         const size_t cps = (size_t)h->nz * (h->chi_has_v ? h->nv : 1);
         for (int s0 = 0; s0 < nslab; s0 += h->nss) {
             const int ns = (nslab - s0 < h->nss) ? nslab - s0 : h->nss;
-            n += 2 * (int)((cps * ns + (size_t)h->nbz - 1) / (size_t)h->nbz) + 1;
+            n += (h->fk.chiv ? 0 : (h->em ? 4 : 2) * (int)((cps * ns + (size_t)h->nbz - 1) / (size_t)h->nbz)) + 1;
         }
         return n;
     }

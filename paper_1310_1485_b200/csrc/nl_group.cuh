@@ -119,12 +119,17 @@ struct Grouped {
 // grid = groups * G CTAs (cooperative launch: every CTA is resident).  scratch: groups * GROUP_SCRATCH_CPLX values;
 // cnt: 2 * groups counters, zeroed before the launch.  chi: the spectral chi planes when CHIV (laid out like g), else
 // unused; R: the real-space chi rows when !CHIV, else unused.
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV>
+// EM (!CHIV only): chi = phi_bar - v_par A_par_bar composed in real space, by linearity: R holds the
+// real-space fields of phi_bar, R2 those of A_par_bar (one plane per (z, slab) each), vp[v + nv * species] the v_par
+// coefficients; slab sl of the launch is global slab slab0 + sl = w + nw * species.
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false>
 __global__ void __launch_bounds__(32 * NW, 1)
 k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R, const cplx* __restrict__ chi,
               const cplx* __restrict__ twx_g, const cplx* __restrict__ twy_g, cplx* __restrict__ scratch,
-              unsigned* __restrict__ cnt, int nz, int nv, int nslab, double kxmin, double kymin, double coef)
+              unsigned* __restrict__ cnt, int nz, int nv, int nslab, double kxmin, double kymin, double coef,
+              const cplx* __restrict__ R2 = nullptr, const double* __restrict__ vp = nullptr, int nw = 1, int slab0 = 0)
 {
+    static_assert(!(EM && CHIV), "the composition needs chi-like fields shared over v");
     using K = Grouped<AX, BX, AY, G, NW, NH, CHIV>;
     constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR, NF = K::NF;
     constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT, UPC = K::UPC, UPP = K::UPP;
@@ -185,6 +190,9 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         const size_t q = (size_t)((t / (unsigned)nv) % (unsigned)nz) + (size_t)nz * (size_t)(t / ((unsigned)nv * (unsigned)nz));
         cplx* Rb = rhs + p * plane_elems;
         [[maybe_unused]] const cplx* Rc = CHIV ? nullptr : R + q * ((size_t)NX * NY);
+        [[maybe_unused]] const cplx* Rc2 = EM ? R2 + q * ((size_t)NX * NY) : nullptr;
+        [[maybe_unused]] double vpar = 0.0;
+        if constexpr (EM) vpar = __ldg(vp + (t % (unsigned)nv) + (unsigned)nv * (((unsigned)slab0 + t / ((unsigned)nv * (unsigned)nz)) / (unsigned)nw));
 
         // =============== X1: derivative, pad, x-synthesis of this CTA's column units; rows go to Z ===============
 #pragma unroll 1
@@ -300,6 +308,19 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
                 }
             };
+            // (dx chi, dy chi) of row `row` at y = k1 + AY k2, k2 < 8, from the real-space rows (EM: composed from two fields)
+            auto load_chi = [&](cplx (&c)[8], int row, int k1) {
+                const size_t off = (size_t)row * NY + k1;
+#pragma unroll
+                for (int k2 = 0; k2 < 8; ++k2) c[k2] = ldg_nc_early(Rc + off + AY * k2);
+                if constexpr (EM) {
+#pragma unroll
+                    for (int k2 = 0; k2 < 8; ++k2) {
+                        const cplx a2 = ldg_nc_early(Rc2 + off + AY * k2);
+                        c[k2] = cmake(fma(-vpar, a2.x, c[k2].x), fma(-vpar, a2.y, c[k2].y));
+                    }
+                }
+            };
 #pragma unroll 1
             for (int item = warp; item < K::NITEM; item += NW) {
                 const int q0 = rank * PPG + item * NPW;           // first pair of the item
@@ -312,11 +333,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                                       (uint32_t)(2 * W2 * sizeof(cplx)), ybar, pol_keep);
                 }
                 [[maybe_unused]] cplx chv[8];
-                if constexpr (!CHIV && !(((NPW * AY + 31) / 32) < NPW)) {   // (flat items: requested after the wait, below)
-                    const cplx* Rr = Rc + (size_t)q0 * NY + k1y;
-#pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
-                }
+                if constexpr (!CHIV && !(((NPW * AY + 31) / 32) < NPW)) load_chi(chv, q0, k1y);   // (flat items: below)
                 mbar_wait(ybar, yph);
                 yph ^= 1;
                 // Y2 items (pair j, k1): NPW AY of them.  With AY lanes per pair a round is one pair (AY of 32 lanes busy);
@@ -342,9 +359,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 if constexpr (FLAT && !CHIV) {   // the first round's chi values for the flat item of this lane
                     int j, k1; bool valid;
                     item_of(0, j, k1, valid);
-                    const cplx* Rr = Rc + (size_t)(q0 + j) * NY + k1;
-#pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) chv[k2] = ldg_nc_early(Rr + AY * k2);
+                    load_chi(chv, q0 + j, k1);
                 }
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
@@ -363,9 +378,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                             if (!(h == 1 && r + 1 == NR)) {
                                 int jn, k1n; bool vn;
                                 item_of(rn, jn, k1n, vn);
-                                const cplx* Rr = Rc + (size_t)(q0 + jn + hn * NPAIR) * NY + k1n;
-#pragma unroll
-                                for (int k2 = 0; k2 < 8; ++k2) chn[k2] = ldg_nc_early(Rr + AY * k2);
+                                load_chi(chn, q0 + jn + hn * NPAIR, k1n);
                             }
                         }
                         [[maybe_unused]] cplx tqr[8];

@@ -37,12 +37,14 @@ def composed_chi(wl, phi, apar, vpar):
     return chi
 
 
-def run_em(wl, phi, apar, vpar, g, rhs, scratch_bytes=None, host=False):
+def run_em(wl, phi, apar, vpar, g, rhs, scratch_bytes=None, host=False, plane_kernel=None):
     from paper_1310_1485_b200 import (GENE_NL_CHI_EM, gene_nl_compute_em, gene_nl_compute_em_host, gene_nl_create,
-                                      gene_nl_destroy, gene_nl_set_scratch_bytes)
+                                      gene_nl_destroy, gene_nl_set_plane_kernel, gene_nl_set_scratch_bytes)
     out = rhs.clone()
     h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
     try:
+        if plane_kernel is not None:
+            gene_nl_set_plane_kernel(h, plane_kernel)
         if scratch_bytes is not None:
             gene_nl_set_scratch_bytes(h, scratch_bytes)
         if host:
@@ -58,16 +60,20 @@ def run_em(wl, phi, apar, vpar, g, rhs, scratch_bytes=None, host=False):
     return out
 
 
-SHAPES = [(16, 8, 3, 5, 2, 2), (64, 32, 2, 3, 2, 1), (96, 48, 2, 4, 1, 2), (128, 32, 3, 3, 1, 1), (256, 64, 2, 2, 1, 2),
+SHAPES = [(16, 8, 3, 5, 2, 2), (64, 32, 2, 3, 2, 1), (96, 48, 2, 4, 1, 2), (96, 48, 3, 5, 3, 2), (128, 32, 3, 3, 1, 1),
+          (256, 64, 2, 2, 1, 2), (256, 64, 2, 3, 3, 2),
           (32, 128, 1, 3, 1, 1),
           (256, 64, 36, 2, 1, 1)]   # chi rows of a chunk beyond 40 MB: k_ybracket<EM> walks its tiles v-fastest
 
 
+# the composition runs in the group kernel where one exists (144 x 144 and 384 x 192 planes), else in k_ybracket<EM>;
+# kind 3 = GENE_NL_KERNEL_BATCHED forces the latter everywhere
+@pytest.mark.parametrize("kind", [None, 3])
 @pytest.mark.parametrize("nx0,nky0,nz,nv,nw,nspec", SHAPES)
-def test_em_matches_oracle_on_composed_chi(cuda_device, nx0, nky0, nz, nv, nw, nspec):
+def test_em_matches_oracle_on_composed_chi(cuda_device, nx0, nky0, nz, nv, nw, nspec, kind):
     wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, False, seed=200 + nx0 + nky0)
     phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
-    out = run_em(wl, phi, apar, vpar, g, rhs)
+    out = run_em(wl, phi, apar, vpar, g, rhs, plane_kernel=kind)
     chi = composed_chi(wl, phi, apar, vpar)
     G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
     ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
@@ -94,15 +100,16 @@ def test_em_under_a_tiny_scratch_budget_and_against_the_per_plane_chi_path(cuda_
 def test_em_host_entry_point_matches_the_device_entry_point(cuda_device):
     """gene_nl_compute_em_host streams (w,s) slabs through the same kernels: the same bits as gene_nl_compute_em; the
     species index of a slab (v_par is per species) must survive the slab-by-slab walk."""
-    wl = W.small_workload(64, 32, 3, 4, 3, 2, 0.05, 0.05, False, seed=33)
-    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
-    dev = run_em(wl, phi, apar, vpar, g, rhs)
-    hst = run_em(wl, phi, apar, vpar, g, rhs, host=True)
-    assert torch.equal(dev, hst)
-    chi = composed_chi(wl, phi, apar, vpar)
-    G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
-    ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
-    assert plane_errors(wl, W.as_planes(hst, wl).cpu().numpy(), ref, R).max() <= TOL
+    for nx0, nky0 in ((64, 32), (96, 48)):     # batched kernels / group kernel behind the streaming driver
+        wl = W.small_workload(nx0, nky0, 3, 4, 3, 2, 0.05, 0.05, False, seed=33)
+        phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+        dev = run_em(wl, phi, apar, vpar, g, rhs)
+        hst = run_em(wl, phi, apar, vpar, g, rhs, host=True)
+        assert torch.equal(dev, hst)
+        chi = composed_chi(wl, phi, apar, vpar)
+        G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
+        ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
+        assert plane_errors(wl, W.as_planes(hst, wl).cpu().numpy(), ref, R).max() <= TOL
 
 
 def test_em_errors(cuda_device):
