@@ -76,22 +76,23 @@ __device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uin
 // NH: k1 passes of the X1 exchange tile (2: half of the k1 range at a time, for AX = 24; 1 for AX = 12).
 // CHIV: chi per plane (chi_has_v = 1): chi goes through X1 like g and its rows are transformed next to those of g in Y
 // (no real-space chi array R); else chi is shared over v and its real-space rows (dx chi, dy chi) come from R.
-template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_>
+// BY: radix of the second y stage (Ny = AY * BY; 8, or 16 for Ny = 384); NPW: row pairs per warp item (NPW * BY <= 32).
+template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_, int BY_ = 8, int NPW_ = 3>
 struct Grouped {
-    static constexpr int AX = AX_, BX = BX_, AY = AY_, G = G_, NW = NW_, NH = NH_;
+    static constexpr int AX = AX_, BX = BX_, AY = AY_, G = G_, NW = NW_, NH = NH_, BY = BY_, BYP = BY_ + 1;
     static constexpr bool CHIV = CHIV_;
     static constexpr int NF = CHIV ? 2 : 1;            // fields that go through X1 and the row hand-over
-    static constexpr int NX = AX * BX, NY = 8 * AY, C2 = BX / 2;
+    static constexpr int NX = AX * BX, NY = BY * AY, C2 = BX / 2;
     static constexpr int NKY0 = NY / 3, W2 = 2 * NKY0, NPAIR = NX / 2;
     static constexpr int M = NX / 3, NX0 = 2 * M;
     static constexpr int CK = 8;                       // stored columns per unit: 128 B runs in both hand-overs
     static constexpr int NUNIT = NKY0 / CK;            // column units per plane
     static constexpr int UPC = NUNIT / G_;             // column units per CTA
     static constexpr int PPG = NPAIR / G;              // row pairs per CTA
-    static constexpr int NPW = 3;                      // row pairs per warp item
+    static constexpr int NPW = NPW_;                   // row pairs per warp item
     static constexpr int NITEM = PPG / NPW;            // items per CTA
     static constexpr int NT = 32 * NW;
-    static constexpr int FY = AY * 9;                  // y exchange tile of one row: [k1][9]
+    static constexpr int FY = AY * BYP;                // y exchange tile of one row: [k1][BY + 1]
     static constexpr int PS = (W2 + FY) | 1;           // pair storage: rows m + NX/2 | m, the tile over row m and beyond
     static constexpr int YB_CPLX = NW * NF * NPW * PS;
     static constexpr int BPX = Tile<AX, BX>::BP, AXH = AX / NH;
@@ -99,20 +100,24 @@ struct Grouped {
     static constexpr int E_CPLX = 2 * CK * CSH;        // X1: both signs of a unit's columns, AXH values of k1 at a time
     static constexpr int CSF = Tile<AX, BX>::STRIDE;
     static constexpr int XBIG = AX > BX ? AX : BX;
-    static constexpr int UPP = (NT / (CK * XBIG)) < UPC ? (NT / (CK * XBIG)) : UPC;   // X2: units per pass
+    static constexpr int UPP0 = NT / (CK * XBIG);
+    static constexpr int UPP = UPP0 < 1 ? 1 : (UPP0 < UPC ? UPP0 : UPC);   // X2: units per pass
     static constexpr int TX_CPLX = UPP * CK * CSF;     // X2: exchange tiles of the units of one pass
     static constexpr int XR_CPLX = E_CPLX > TX_CPLX ? E_CPLX : TX_CPLX;
-    static constexpr int A_CPLX = YB_CPLX > XR_CPLX ? YB_CPLX : XR_CPLX;   // the x tiles and the y pair storages share a region
     static constexpr int G_CPLX = CK * NX0;            // one unit's columns of a spectral plane (one contiguous block)
-    static constexpr int TWX = AX * BPX, TWY = AY * 9;
+    // One region A serves the phases in turn: X1 (E at 0, the staged column block behind the x tiles), Y (the warps'
+    // pair storages: no block is in flight then), X2 (Tx at 0, the next plane's first block behind it).
+    static constexpr int GS_OFF = XR_CPLX;
+    static constexpr int A_CPLX = YB_CPLX > GS_OFF + G_CPLX ? YB_CPLX : GS_OFF + G_CPLX;
+    static constexpr int TWX = AX * BPX, TWY = AY * BYP;
     static constexpr int NBAR = 1 + NW;                // mbarriers: column block, rows of each warp
-    static constexpr int SMEM_CPLX = A_CPLX + G_CPLX + TWX + TWY + (NBAR + 1) / 2;
+    static constexpr int SMEM_CPLX = A_CPLX + TWX + TWY + (NBAR + 1) / 2;
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
     static constexpr size_t ZS_CPLX = (size_t)NPAIR * 2 * W2, PS_CPLX = (size_t)NPAIR * W2;   // per-group scratch
     static constexpr size_t GROUP_SCRATCH_CPLX = NF * ZS_CPLX + PS_CPLX;
     static_assert(AX % 3 == 0 && AY % 3 == 0 && AX % NH == 0 && BX % 2 == 0, "3/2 rule; k1 passes; row pairs");
     static_assert(NKY0 % CK == 0 && NUNIT % G == 0 && NPAIR % G == 0 && PPG % NPW == 0, "the group divides the work");
-    static_assert(NPW * 8 <= 32 && AY <= 32 && NKY0 == 8 * (AY / 3), "lanes of the y stages");
+    static_assert(NPW * BY <= 32 && AY <= 32 && NKY0 == BY * (AY / 3) && (BY == 8 || BY == 16), "lanes of the y stages");
     static_assert(2 * CK * BX <= NT && 2 * CK * AXH <= NT && UPP >= 1 && UPC % UPP == 0, "one item per thread in every x stage");
 };
 
@@ -122,7 +127,7 @@ struct Grouped {
 // EM (!CHIV only): chi = phi_bar - v_par A_par_bar composed in real space, by linearity: R holds the
 // real-space fields of phi_bar, R2 those of A_par_bar (one plane per (z, slab) each), vp[v + nv * species] the v_par
 // coefficients; slab sl of the launch is global slab slab0 + sl = w + nw * species.
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false>
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW_ = 3>
 __global__ void __launch_bounds__(32 * NW, 1)
 k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R, const cplx* __restrict__ chi,
               const cplx* __restrict__ twx_g, const cplx* __restrict__ twy_g, cplx* __restrict__ scratch,
@@ -130,7 +135,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
               const cplx* __restrict__ R2 = nullptr, const double* __restrict__ vp = nullptr, int nw = 1, int slab0 = 0)
 {
     static_assert(!(EM && CHIV), "the composition needs chi-like fields shared over v");
-    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV>;
+    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW_>;
+    constexpr int BYP = K::BYP;
     constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR, NF = K::NF;
     constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT, UPC = K::UPC, UPP = K::UPP;
     constexpr int PS = K::PS, BPX = K::BPX, CSH = K::CSH, CSF = K::CSF, AXH = K::AXH;
@@ -140,9 +146,9 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
 
     extern __shared__ cplx smem[];
     cplx* A = smem;                        // X1: E / X2: Tx / Y: pair storages of the warps
-    cplx* Gs = A + K::A_CPLX;              // a unit's columns of g or chi (bulk copy)
-    cplx* twx = Gs + K::G_CPLX;            // W_NX^{n2 k1}, [k1][BPX]
-    cplx* twy = twx + K::TWX;              // W_NY^{k1 k2}, [k1][9]
+    cplx* Gs = A + K::GS_OFF;              // a unit's columns of g or chi (bulk copy), behind the x tiles
+    cplx* twx = A + K::A_CPLX;             // W_NX^{n2 k1}, [k1][BPX]
+    cplx* twy = twx + K::TWX;              // W_NY^{k1 k2}, [k1][BY + 1]
     const uint32_t bars = smem_u32(twy + K::TWY);
     const uint32_t gbar = bars;
 
@@ -157,7 +163,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
     unsigned* pcnt = zcnt + 1;
 
     load_twiddles_ab<AX, BX>(twx, twx_g);
-    load_twiddles_ab<AY, 8>(twy, twy_g);
+    load_twiddles_ab<AY, BY>(twy, twy_g);
     if (tid == 0) {
         mbar_init(gbar, 1);
         for (int w = 0; w < NW; ++w) mbar_init(bars + 8 + 8 * w, 1);
@@ -236,10 +242,9 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 }
             }
             __syncthreads();   // every thread has read its values of the block
-            if (tid == 0) {    // the next block: the next step of this plane, or the first step of the next plane
-                if (s + 1 < NF * UPC) request_block(t, s + 1);
-                else if (t + (unsigned)ngroup < T) request_block(t + (unsigned)ngroup, 0);
-            }
+            // the next step's block (the first block of the next plane is requested when X2 starts: region A holds
+            // the pair storages in between)
+            if (tid == 0 && s + 1 < NF * UPC) request_block(t, s + 1);
 #pragma unroll
             for (int hk = 0; hk < K::NH; ++hk) {
                 if (has1) {
@@ -282,13 +287,16 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
             const int lane = opaque(lane0);
             const int k1y = lane < AY ? lane : lane - AY;   // lanes >= AY shadow an item (same addresses) and skip the stores
             const bool act2 = lane < AY;
-            const int j1 = (lane >> 3) < NPW ? (lane >> 3) : 0;   // Y1 / Y3 item: pair j1 of the warp item, position lane & 7
-            const bool act1 = (lane >> 3) < NPW;
-            const int n2 = lane & 7;
+            const int j1 = (lane / BY) < NPW ? (lane / BY) : 0;   // Y1 / Y3 item: pair j1 of the warp item, position lane mod BY
+            const bool act1 = (lane / BY) < NPW;
+            const int n2 = lane % BY;
+            constexpr bool TWREG = (BY == 8);                     // the lane's y twiddles in registers (else read at every use)
             cplx* Zw = A + (warp * NF * NPW) * PS;                // this warp's pair storages: g, then (CHIV) chi
-            cplx tq[8];
+            [[maybe_unused]] cplx tq[BY];
+            if constexpr (TWREG) {
 #pragma unroll
-            for (int k2 = 1; k2 < 8; ++k2) tq[k2] = twy[k1y * 9 + k2];
+                for (int k2 = 1; k2 < BY; ++k2) tq[k2] = twy[k1y * BYP + k2];
+            }
             // Y1: pruned radix-AY of rows m (h = 0: second half of the storage) / m + NX/2 (h = 1: first half) of the NPW
             // pairs that start at storage Zst; the exchange tile of a pair starts at its row m
             auto y1 = [&](cplx* Zst, int h) {
@@ -296,8 +304,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 cplx lo[AY1], hi[AY1];
 #pragma unroll
                 for (int a = 0; a < AY1; ++a) {
-                    lo[a] = Zr[8 * a];
-                    hi[a] = Zr[8 * a + NKY0];
+                    lo[a] = Zr[BY * a];
+                    hi[a] = Zr[BY * a + NKY0];
                 }
                 cplx out[AY];
                 dft_pruned_in<AY, +1>(lo, hi, out);
@@ -305,17 +313,17 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 if (act1) {
                     cplx* tile = Zst + j1 * PS + W2 + n2;
 #pragma unroll
-                    for (int k1 = 0; k1 < AY; ++k1) tile[k1 * 9] = out[k1];
+                    for (int k1 = 0; k1 < AY; ++k1) tile[k1 * BYP] = out[k1];
                 }
             };
             // (dx chi, dy chi) of row `row` at y = k1 + AY k2, k2 < 8, from the real-space rows (EM: composed from two fields)
-            auto load_chi = [&](cplx (&c)[8], int row, int k1) {
+            auto load_chi = [&](cplx (&c)[BY], int row, int k1) {
                 const size_t off = (size_t)row * NY + k1;
 #pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) c[k2] = ldg_nc_early(Rc + off + AY * k2);
+                for (int k2 = 0; k2 < BY; ++k2) c[k2] = ldg_nc_early(Rc + off + AY * k2);
                 if constexpr (EM) {
 #pragma unroll
-                    for (int k2 = 0; k2 < 8; ++k2) {
+                    for (int k2 = 0; k2 < BY; ++k2) {
                         const cplx a2 = ldg_nc_early(Rc2 + off + AY * k2);
                         c[k2] = cmake(fma(-vpar, a2.x, c[k2].x), fma(-vpar, a2.y, c[k2].y));
                     }
@@ -332,7 +340,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                         bulk_g2s_hint(smem_u32(Zw + j * PS), Zs + (size_t)(j / NPW) * K::ZS_CPLX + (size_t)(q0 + j % NPW) * (2 * W2),
                                       (uint32_t)(2 * W2 * sizeof(cplx)), ybar, pol_keep);
                 }
-                [[maybe_unused]] cplx chv[8];
+                [[maybe_unused]] cplx chv[BY];
                 if constexpr (!CHIV && !(((NPW * AY + 31) / 32) < NPW)) load_chi(chv, q0, k1y);   // (flat items: below)
                 mbar_wait(ybar, yph);
                 yph ^= 1;
@@ -342,7 +350,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 constexpr int NY2 = NPW * AY, NRF = (NY2 + 31) / 32;
                 constexpr bool FLAT = NRF < NPW;
                 constexpr int NR = FLAT ? NRF : NPW;
-                double nlx[NR][8];                                    // bracket of the rows m (first halves), kept in registers
+                constexpr bool AHEAD = (BY == 8);                     // chi values of the next round in a second register set
+                double nlx[NR][BY];                                   // bracket of the rows m (first halves), kept in registers
                 auto item_of = [&](int r, int& j, int& k1, bool& valid) {
                     if constexpr (FLAT) {
                         const int idx = r * 32 + lane;
@@ -370,55 +379,71 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     for (int r = 0; r < NR; ++r) {  // Y2: twiddle + radix-8 to real space, bracket
                         int j, k1; bool valid;
                         item_of(r, j, k1, valid);
-                        [[maybe_unused]] cplx chn[8];
-                        if constexpr (!CHIV) {
-                            // chi values of the NEXT round (or of the first round of the second half), requested before
-                            // this round's butterflies so that their latency hides behind them
+                        // chi values of the NEXT round (or of the first round of the second half): requested before this
+                        // round's butterflies (AHEAD: into a second register set) or right after this round's bracket
+                        auto next_chi = [&](cplx (&dst)[BY]) {
                             const int rn = (r + 1 < NR) ? r + 1 : 0, hn = (r + 1 < NR) ? h : 1;
                             if (!(h == 1 && r + 1 == NR)) {
                                 int jn, k1n; bool vn;
                                 item_of(rn, jn, k1n, vn);
-                                load_chi(chn, q0 + jn + hn * NPAIR, k1n);
+                                load_chi(dst, q0 + jn + hn * NPAIR, k1n);
                             }
-                        }
+                        };
+                        [[maybe_unused]] cplx chn[AHEAD ? BY : 1];
+                        if constexpr (!CHIV && AHEAD) next_chi(chn);
+                        const cplx* twl = twy + k1 * BYP;   // the item's twiddles W_NY^{k1 k2} (when they are not in registers)
                         [[maybe_unused]] cplx tqr[8];
-                        if constexpr (FLAT) {
+                        if constexpr (FLAT && BY == 8) {
 #pragma unroll
-                            for (int k2 = 1; k2 < 8; ++k2) tqr[k2] = twy[k1 * 9 + k2];
+                            for (int k2 = 1; k2 < 8; ++k2) tqr[k2] = twl[k2];
                         }
-                        const cplx (&tw)[8] = *(FLAT ? &tqr : &tq);
-                        cplx* tile = Zw + j * PS + W2 + k1 * 9;
-                        cplx v[8];
+                        // twiddle + radix-BY to real space
+                        auto to_real = [&](cplx (&x)[BY]) {
+                            if constexpr (BY == 8) {
+                                if constexpr (FLAT) dft8_twiddled<+1>(x, tqr); else dft8_twiddled<+1>(x, tq);
+                            } else {
 #pragma unroll
-                        for (int i = 0; i < 8; ++i) v[i] = tile[i];
-                        dft8_twiddled<+1>(v, tw);   // (dx g + i dy g)(row, y = k1 + AY k2)
+                                for (int i = 1; i < BY; ++i) { const cplx w = twl[i]; x[i] = cmul(x[i], w.x, w.y); }
+                                Dft<BY, +1>::run(x);
+                            }
+                        };
+                        cplx* tile = Zw + j * PS + W2 + k1 * BYP;
+                        cplx v[BY];
+#pragma unroll
+                        for (int i = 0; i < BY; ++i) v[i] = tile[i];
+                        to_real(v);                 // (dx g + i dy g)(row, y = k1 + AY k2)
                         if constexpr (CHIV) {       // (dx chi + i dy chi) of the same row from chi's tile
-                            const cplx* tc = Zw + (NPW + j) * PS + W2 + k1 * 9;
+                            const cplx* tc = Zw + (NPW + j) * PS + W2 + k1 * BYP;
 #pragma unroll
-                            for (int i = 0; i < 8; ++i) chv[i] = tc[i];
-                            dft8_twiddled<+1>(chv, tw);
+                            for (int i = 0; i < BY; ++i) chv[i] = tc[i];
+                            to_real(chv);
                         }
                         if (h == 0) {
 #pragma unroll
-                            for (int k2 = 0; k2 < 8; ++k2) nlx[r][k2] = fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x);
+                            for (int k2 = 0; k2 < BY; ++k2) nlx[r][k2] = fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x);
+                            if constexpr (!CHIV && !AHEAD) next_chi(chv);
                         } else {
-                            cplx w[8];
+                            cplx w[BY];
 #pragma unroll
-                            for (int k2 = 0; k2 < 8; ++k2)
+                            for (int k2 = 0; k2 < BY; ++k2)
                                 w[k2] = cmake(nlx[r][k2], fma(chv[k2].x, v[k2].y, -chv[k2].y * v[k2].x));
-                            Dft<8, -1>::run(w);
+                            if constexpr (!CHIV && !AHEAD) next_chi(chv);
+                            Dft<BY, -1>::run(w);
 #pragma unroll
-                            for (int k2 = 1; k2 < 8; ++k2) w[k2] = cmul(w[k2], tw[k2].x, -tw[k2].y);
-                            if constexpr (FLAT) __syncwarp(FULL);   // shadow lanes have read their tiles before the owners overwrite them
+                            for (int k2 = 1; k2 < BY; ++k2) {
+                                cplx t;
+                                if constexpr (BY == 8) t = FLAT ? tqr[k2] : tq[k2]; else t = twl[k2];
+                                w[k2] = cmul(w[k2], t.x, -t.y);
+                            }
                             if (valid) {  // own slots of the tile: no other active lane reads or writes them in this phase
 #pragma unroll
-                                for (int k2 = 0; k2 < 8; ++k2) tile[k2] = w[k2];
+                                for (int k2 = 0; k2 < BY; ++k2) tile[k2] = w[k2];
                             }
                         }
-                        if constexpr (!CHIV) {
+                        if constexpr (!CHIV && AHEAD) {
                             if (!(h == 1 && r + 1 == NR)) {
 #pragma unroll
-                                for (int k2 = 0; k2 < 8; ++k2) chv[k2] = chn[k2];
+                                for (int k2 = 0; k2 < BY; ++k2) chv[k2] = chn[k2];
                             }
                         }
                     }
@@ -428,15 +453,15 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     const cplx* tile = Zw + j1 * PS + W2 + n2;
                     cplx in[AY];
 #pragma unroll
-                    for (int n1 = 0; n1 < AY; ++n1) in[n1] = tile[n1 * 9];
+                    for (int n1 = 0; n1 < AY; ++n1) in[n1] = tile[n1 * BYP];
                     cplx lo[AY1], hi[AY1];
                     dft_pruned_out<AY, -1>(in, lo, hi);
                     if (act1) {
                         cplx* Pp = Ps + (size_t)(q0 + j1) * W2 + n2;
 #pragma unroll
                         for (int c = 0; c < AY1; ++c) {
-                            stg_hint(Pp + 8 * c, lo[c], pol_keep);          // +ky half: cc = ky = n2 + 8 c
-                            stg_hint(Pp + 8 * c + NKY0, hi[c], pol_keep);   // -ky half: cc = nky0 + n2 + 8 c  <->  ky = nky0 - n2 - 8 c
+                            stg_hint(Pp + BY * c, lo[c], pol_keep);          // +ky half: cc = ky = n2 + BY c
+                            stg_hint(Pp + BY * c + NKY0, hi[c], pol_keep);   // -ky half: cc = nky0 + n2 + BY c  <->  ky = nky0 - n2 - BY c
                         }
                     }
                 }
@@ -453,6 +478,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         __syncthreads();
 
         // =============== X2: x-analysis of this CTA's column units, UPP at a time; delete modes, prefactor, add ===============
+        if (tid == 0 && t + (unsigned)ngroup < T) request_block(t + (unsigned)ngroup, 0);   // lands behind the x tiles
         {
             cplx r0[AX1], r1[AX1];
             const int k2s = tid % BX, cols = (tid / BX) % CK, us = tid / (BX * CK);   // stage 2 item: (unit us of the pass, column, k2)
