@@ -80,12 +80,12 @@ FusedKernel make_cluster()
     return k;
 }
 
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW = 3>
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW = 3, int AX2 = 0, int BX2 = 0>
 FusedKernel make_group()
 {
-    using K = gnl::Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW>;
+    using K = gnl::Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW, AX2, BX2>;
     FusedKernel k;
-    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV, EM, BY, NPW>;
+    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV, EM, BY, NPW, AX2, BX2>;
     k.chiv = CHIV;
     k.group = G;
     k.group_scratch = sizeof(cplx) * K::GROUP_SCRATCH_CPLX;
@@ -103,7 +103,7 @@ bool find_group(int nx, int ny, bool chi_has_v, bool em, FusedKernel* out)
         return false;
     }
     if (nx == 384 && ny == 192 && !chi_has_v) { *out = make_group<24, 16, 24, 4, 8, 2, false>(); return out->smem <= 227 * 1024; }
-    if (nx == 768 && ny == 384 && !chi_has_v) { *out = make_group<48, 16, 24, 8, 8, 4, false, false, 16, 2>(); return out->smem <= 227 * 1024; }
+    if (nx == 768 && ny == 384 && !chi_has_v) { *out = make_group<48, 16, 24, 8, 8, 4, false, false, 16, 2, 24, 32>(); return out->smem <= 227 * 1024; }
     if (nx == 144 && ny == 144 && chi_has_v) { *out = make_group<12, 12, 18, 1, 8, 1, true>(); return out->smem <= 227 * 1024; }
     if (nx == 144 && ny == 144 && !chi_has_v) { *out = make_group<12, 12, 18, 1, 8, 1, false>(); return out->smem <= 227 * 1024; }
     return false;

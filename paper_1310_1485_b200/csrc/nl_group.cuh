@@ -77,8 +77,12 @@ __device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uin
 // CHIV: chi per plane (chi_has_v = 1): chi goes through X1 like g and its rows are transformed next to those of g in Y
 // (no real-space chi array R); else chi is shared over v and its real-space rows (dx chi, dy chi) come from R.
 // BY: radix of the second y stage (Ny = AY * BY; 8, or 16 for Ny = 384); NPW: row pairs per warp item (NPW * BY <= 32).
-template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_, int BY_ = 8, int NPW_ = 3>
+// AX2 x BX2: the split of Nx used by the x-analysis (X2) when it differs from the synthesis' (768 = 48 x 16 on the way in,
+// 24 x 32 on the way back: every thread has an item in the stage that carries the pruned radix).
+template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_, int BY_ = 8, int NPW_ = 3, int AX2_ = 0, int BX2_ = 0>
 struct Grouped {
+    static constexpr int AX2 = AX2_ ? AX2_ : AX_, BX2 = BX2_ ? BX2_ : BX_, C22 = BX2 / 2;
+    static constexpr int BPX2 = Tile<AX2, BX2>::BP;
     static constexpr int AX = AX_, BX = BX_, AY = AY_, G = G_, NW = NW_, NH = NH_, BY = BY_, BYP = BY_ + 1;
     static constexpr bool CHIV = CHIV_;
     static constexpr int NF = CHIV ? 2 : 1;            // fields that go through X1 and the row hand-over
@@ -98,8 +102,8 @@ struct Grouped {
     static constexpr int BPX = Tile<AX, BX>::BP, AXH = AX / NH;
     static constexpr int CSH = ((AXH * BPX) | 1) + ((((AXH * BPX) | 1) % 8 == 1) ? 4 : 0);   // tile of one column-sign, AXH values of k1
     static constexpr int E_CPLX = 2 * CK * CSH;        // X1: both signs of a unit's columns, AXH values of k1 at a time
-    static constexpr int CSF = Tile<AX, BX>::STRIDE;
-    static constexpr int XBIG = AX > BX ? AX : BX;
+    static constexpr int CSF = Tile<AX2, BX2>::STRIDE;
+    static constexpr int XBIG = AX2 > BX2 ? AX2 : BX2;
     static constexpr int UPP0 = NT / (CK * XBIG);
     static constexpr int UPP = UPP0 < 1 ? 1 : (UPP0 < UPC ? UPP0 : UPC);   // X2: units per pass
     static constexpr int TX_CPLX = UPP * CK * CSF;     // X2: exchange tiles of the units of one pass
@@ -110,8 +114,9 @@ struct Grouped {
     static constexpr int GS_OFF = XR_CPLX;
     static constexpr int A_CPLX = YB_CPLX > GS_OFF + G_CPLX ? YB_CPLX : GS_OFF + G_CPLX;
     static constexpr int TWX = AX * BPX, TWY = AY * BYP;
+    static constexpr int TWX2 = (AX2 == AX && BX2 == BX) ? 0 : AX2 * BPX2;   // X2's own twiddle table when its split differs
     static constexpr int NBAR = 1 + NW;                // mbarriers: column block, rows of each warp
-    static constexpr int SMEM_CPLX = A_CPLX + TWX + TWY + (NBAR + 1) / 2;
+    static constexpr int SMEM_CPLX = A_CPLX + TWX + TWX2 + TWY + (NBAR + 1) / 2;
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
     static constexpr size_t ZS_CPLX = (size_t)NPAIR * 2 * W2, PS_CPLX = (size_t)NPAIR * W2;   // per-group scratch
     static constexpr size_t GROUP_SCRATCH_CPLX = NF * ZS_CPLX + PS_CPLX;
@@ -119,6 +124,7 @@ struct Grouped {
     static_assert(NKY0 % CK == 0 && NUNIT % G == 0 && NPAIR % G == 0 && PPG % NPW == 0, "the group divides the work");
     static_assert(NPW * BY <= 32 && AY <= 32 && NKY0 == BY * (AY / 3) && (BY == 8 || BY == 16), "lanes of the y stages");
     static_assert(2 * CK * BX <= NT && 2 * CK * AXH <= NT && UPP >= 1 && UPC % UPP == 0, "one item per thread in every x stage");
+    static_assert(AX2 * BX2 == NX && AX2 % 3 == 0 && BX2 % 2 == 0 && UPP * CK * BX2 <= NT, "the x-analysis split");
 };
 
 // grid = groups * G CTAs (cooperative launch: every CTA is resident).  scratch: groups * GROUP_SCRATCH_CPLX values;
@@ -127,7 +133,7 @@ struct Grouped {
 // EM (!CHIV only): chi = phi_bar - v_par A_par_bar composed in real space, by linearity: R holds the
 // real-space fields of phi_bar, R2 those of A_par_bar (one plane per (z, slab) each), vp[v + nv * species] the v_par
 // coefficients; slab sl of the launch is global slab slab0 + sl = w + nw * species.
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW_ = 3>
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW_ = 3, int AX2_ = 0, int BX2_ = 0>
 __global__ void __launch_bounds__(32 * NW, 1)
 k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R, const cplx* __restrict__ chi,
               const cplx* __restrict__ twx_g, const cplx* __restrict__ twy_g, cplx* __restrict__ scratch,
@@ -135,8 +141,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
               const cplx* __restrict__ R2 = nullptr, const double* __restrict__ vp = nullptr, int nw = 1, int slab0 = 0)
 {
     static_assert(!(EM && CHIV), "the composition needs chi-like fields shared over v");
-    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW_>;
-    constexpr int BYP = K::BYP;
+    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW_, AX2_, BX2_>;
+    constexpr int BYP = K::BYP, AX2 = K::AX2, BX2 = K::BX2, C22 = K::C22, BPX2 = K::BPX2, AX21 = K::AX2 / 3;
     constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR, NF = K::NF;
     constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT, UPC = K::UPC, UPP = K::UPP;
     constexpr int PS = K::PS, BPX = K::BPX, CSH = K::CSH, CSF = K::CSF, AXH = K::AXH;
@@ -148,7 +154,8 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
     cplx* A = smem;                        // X1: E / X2: Tx / Y: pair storages of the warps
     cplx* Gs = A + K::GS_OFF;              // a unit's columns of g or chi (bulk copy), behind the x tiles
     cplx* twx = A + K::A_CPLX;             // W_NX^{n2 k1}, [k1][BPX]
-    cplx* twy = twx + K::TWX;              // W_NY^{k1 k2}, [k1][BY + 1]
+    cplx* twx2 = K::TWX2 ? twx + K::TWX : twx;   // W_NX^{n1 k2} of the x-analysis split, [n1][BPX2]
+    cplx* twy = twx + K::TWX + K::TWX2;    // W_NY^{k1 k2}, [k1][BY + 1]
     const uint32_t bars = smem_u32(twy + K::TWY);
     const uint32_t gbar = bars;
 
@@ -163,6 +170,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
     unsigned* pcnt = zcnt + 1;
 
     load_twiddles_ab<AX, BX>(twx, twx_g);
+    if constexpr (K::TWX2 != 0) load_twiddles_ab<AX2, BX2>(twx2, twx_g);
     load_twiddles_ab<AY, BY>(twy, twy_g);
     if (tid == 0) {
         mbar_init(gbar, 1);
@@ -480,54 +488,54 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         // =============== X2: x-analysis of this CTA's column units, UPP at a time; delete modes, prefactor, add ===============
         if (tid == 0 && t + (unsigned)ngroup < T) request_block(t + (unsigned)ngroup, 0);   // lands behind the x tiles
         {
-            cplx r0[AX1], r1[AX1];
-            const int k2s = tid % BX, cols = (tid / BX) % CK, us = tid / (BX * CK);   // stage 2 item: (unit us of the pass, column, k2)
-            const bool has2 = tid < UPP * CK * BX;
+            cplx r0[AX21], r1[AX21];
+            const int k2s = tid % BX2, cols = (tid / BX2) % CK, us = tid / (BX2 * CK);   // stage 2 item: (unit us of the pass, column, k2)
+            const bool has2 = tid < UPP * CK * BX2;
 #pragma unroll 1
             for (int ub = 0; ub < UPC; ub += UPP) {
 #pragma unroll 1
-                for (int i1 = tid; i1 < UPP * CK * AX; i1 += NT) {
-                    // stage 1: unpack the row pair, radix-BX over n2 for fixed n1 (m = n1 + AX n2), twiddle
-                    const int col = i1 % CK, n1 = (i1 / CK) % AX, ul = i1 / (CK * AX);
+                for (int i1 = tid; i1 < UPP * CK * AX2; i1 += NT) {
+                    // stage 1: unpack the row pair, radix-BX2 over n2 for fixed n1 (m = n1 + AX2 n2), twiddle
+                    const int col = i1 % CK, n1 = (i1 / CK) % AX2, ul = i1 / (CK * AX2);
                     const int kyi = (rank + G * (ub + ul)) * CK + col;
                     const int ccm = kyi ? W2 - kyi : 0;
-                    cplx x[BX];
+                    cplx x[BX2];
 #pragma unroll
-                    for (int i = 0; i < C2; ++i) {
-                        const cplx* Pr = Ps + (size_t)(n1 + AX * i) * W2;
+                    for (int i = 0; i < C22; ++i) {
+                        const cplx* Pr = Ps + (size_t)(n1 + AX2 * i) * W2;
                         const cplx pp = ldg_cg_hint(Pr + kyi, pol_keep), pm = ldg_cg_hint(Pr + ccm, pol_keep);
                         x[i] = cmake(pp.x + pm.x, pp.y - pm.y);          // 2 N^_m  = P+ + conj P-
-                        x[i + C2] = cmake(pp.y + pm.y, pm.x - pp.x);     // 2 N^_m' = -i (P+ - conj P-)
+                        x[i + C22] = cmake(pp.y + pm.y, pm.x - pp.x);    // 2 N^_m' = -i (P+ - conj P-)
                     }
-                    Dft<BX, -1>::run(x);
-                    cplx* Ec = A + (ul * CK + col) * CSF + n1 * BPX;
+                    Dft<BX2, -1>::run(x);
+                    cplx* Ec = A + (ul * CK + col) * CSF + n1 * BPX2;
 #pragma unroll
-                    for (int k2 = 0; k2 < BX; ++k2) {
-                        const cplx w = twx[n1 * BPX + k2];
+                    for (int k2 = 0; k2 < BX2; ++k2) {
+                        const cplx w = twx2[n1 * BPX2 + k2];
                         Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], w.x, -w.y);
                     }
                 }
                 cplx* Rcol = Rb + (size_t)((rank + G * (ub + us)) * CK + cols) * NX0 + k2s;
                 if (has2) {  // rhs values of this thread's share of stage 2
 #pragma unroll
-                    for (int c = 0; c < AX1; ++c) {
-                        r0[c] = ldg_early(Rcol + BX * c);
-                        r1[c] = ldg_early(Rcol + BX * c + M);
+                    for (int c = 0; c < AX21; ++c) {
+                        r0[c] = ldg_early(Rcol + BX2 * c);
+                        r1[c] = ldg_early(Rcol + BX2 * c + M);
                     }
                 }
                 __syncthreads();
-                if (has2) {  // stage 2: pruned-output radix-AX over n1 for fixed k2; i = k2 + BX c
-                    cplx in[AX];
+                if (has2) {  // stage 2: pruned-output radix-AX2 over n1 for fixed k2; i = k2 + BX2 c
+                    cplx in[AX2];
                     const cplx* Ec = A + (us * CK + cols) * CSF + k2s;
 #pragma unroll
-                    for (int n1 = 0; n1 < AX; ++n1) in[n1] = Ec[n1 * BPX];
-                    cplx lo[AX1], hi[AX1];
-                    dft_pruned_out<AX, -1>(in, lo, hi);
+                    for (int n1 = 0; n1 < AX2; ++n1) in[n1] = Ec[n1 * BPX2];
+                    cplx lo[AX21], hi[AX21];
+                    dft_pruned_out<AX2, -1>(in, lo, hi);
 #pragma unroll
-                    for (int c = 0; c < AX1; ++c) {
-                        Rcol[BX * c] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));
+                    for (int c = 0; c < AX21; ++c) {
+                        Rcol[BX2 * c] = cmake(fma(coef, lo[c].x, r0[c].x), fma(coef, lo[c].y, r0[c].y));
                         if (c != 0 || k2s != 0)  // i = M is the Nyquist row: untouched (R6)
-                            Rcol[BX * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
+                            Rcol[BX2 * c + M] = cmake(fma(coef, hi[c].x, r1[c].x), fma(coef, hi[c].y, r1[c].y));
                     }
                 }
                 __syncthreads();  // the tiles are consumed before the next pass / the next plane's E overwrites them
