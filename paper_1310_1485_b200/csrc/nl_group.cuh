@@ -57,6 +57,12 @@ __device__ __forceinline__ uint64_t l2_policy_evict_first()
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
+// Drop a 128-byte line from L2 without writing it back: the scratch rows a warp has just pulled into shared memory are
+// dead (the next plane overwrites them in full), so their dirty lines need never reach HBM.
+__device__ __forceinline__ void l2_discard_line(const void* p)
+{
+    asm volatile("discard.global.L2 [%0], 128;" ::"l"(p) : "memory");
+}
 __device__ __forceinline__ void stg_hint(cplx* p, cplx v, uint64_t pol)
 {
     asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
@@ -352,6 +358,16 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 if constexpr (!CHIV && !(((NPW * AY + 31) / 32) < NPW)) load_chi(chv, q0, k1y);   // (flat items: below)
                 mbar_wait(ybar, yph);
                 yph ^= 1;
+                // The rows are in shared memory: their lines in the scratch are dead.  Dropping them pays where the groups'
+                // scratch exceeds what L2 keeps (768 x 384: 81 MB; DRAM writes 69 -> 34 GB per launch, time unchanged);
+                // at 384 x 192 (44 MB, already 1.07 x the algorithmic bytes) it cost 14 % of the time: not done there.
+                if constexpr (K::GROUP_SCRATCH_CPLX * sizeof(cplx) > ((size_t)2 << 20)) {
+                    constexpr int LPB = (int)(2 * W2 * sizeof(cplx) / 128);   // lines per pair block
+                    for (int i = lane; i < NF * NPW * LPB; i += 32) {
+                        const int j = i / LPB;
+                        l2_discard_line(Zs + (size_t)(j / NPW) * K::ZS_CPLX + (size_t)(q0 + j % NPW) * (2 * W2) + (size_t)(i % LPB) * 8);
+                    }
+                }
                 // Y2 items (pair j, k1): NPW AY of them.  With AY lanes per pair a round is one pair (AY of 32 lanes busy);
                 // when fewer rounds of 32 cover all items (AY = 18: 54 items, 2 rounds instead of 3) the items are laid
                 // flat over the lanes and the twiddles of a lane's k1 are read again for every round.
