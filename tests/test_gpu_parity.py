@@ -280,6 +280,46 @@ def test_group_kernel_144x144_planes(cuda_device, nz, nv, nw, nspec, chi_has_v, 
     assert torch.equal(gpu_compute(wl, chi, g, rhs, scale=0.0, plane_kernel=kind), rhs)
 
 
+@pytest.mark.parametrize("nx0,nky0,chi_has_v,kind", [
+    (128, 32, False, None),      # k_plane_fused2: __syncwarp-only chains over in-place tiles, shadow lanes
+    (16, 8, False, None),        # k_plane_fused (first generation)
+    (256, 64, False, 2),         # k_plane_group: hand-overs through L2, counters, bulk copies into live tiles
+    (256, 64, False, 1),         # k_plane_cluster: DSMEM stores + mbarrier transaction counts
+    (96, 48, True, 2),           # k_plane_group with chi per plane (groups of one CTA)
+    (512, 128, False, 2),        # k_plane_group, radix-16 second y stage
+    (256, 64, True, 3),          # batched kernels
+])
+def test_repeated_runs_give_the_same_bits(cuda_device, nx0, nky0, chi_has_v, kind):
+    """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so a data race in the shared-memory /
+    distributed-shared-memory / L2 hand-overs has to show up here: the kernels are deterministic by construction (no
+    atomics on data, fixed summation order), so 24 runs under different co-scheduling -- alone, behind a memory-bound
+    kernel on another stream, with a different number of planes in flight -- must agree with the first one bit for bit,
+    and that one with the oracle."""
+    from paper_1310_1485_b200 import GeneNL
+    wl = W.small_workload(nx0, nky0, 3, 5, 2, 1, 0.04, 0.05, chi_has_v, seed=500 + nx0)
+    chi, g, rhs = W.make_inputs(wl, cuda_device)
+    check_parity(wl, cuda_device, plane_kernel=kind)
+    junk = torch.empty(64 << 20, dtype=torch.float64, device=cuda_device)
+    side = torch.cuda.Stream()
+    with GeneNL(wl, plane_kernel=kind) as nl:
+        first = rhs.clone()
+        nl.compute(chi, g, first)
+        torch.cuda.synchronize()
+        for rep in range(24):
+            out = rhs.clone()
+            if rep % 3 == 1:
+                with torch.cuda.stream(side):
+                    junk.mul_(1.0000001)                 # a bandwidth hog next to the kernels
+            nl.compute(chi, g, out)
+            torch.cuda.synchronize()
+            assert torch.equal(out, first), f"run {rep} differs"
+    half = W.small_workload(nx0, nky0, 3, 5, 1, 1, 0.04, 0.05, chi_has_v, seed=500 + nx0)   # first (w,s) slab only
+    sub, cs, gs, rs = W.shard_arrays(wl, chi, g, rhs, 0, 2)
+    assert sub.planes == half.planes
+    part = gpu_compute(sub, cs.contiguous(), gs.contiguous(), rs.contiguous(), plane_kernel=kind)
+    assert torch.equal(part.reshape(-1), first.reshape(2, -1)[0])
+
+
 def test_config1_sampled_modes_against_the_definition(cuda_device):
     """Sampled outputs the definition can compute one by one, at BASELINE.json's full size."""
     wl = W.CONFIGS[1]
