@@ -80,12 +80,13 @@ FusedKernel make_cluster()
     return k;
 }
 
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW = 3, int AX2 = 0, int BX2 = 0>
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW = 3, int AX2 = 0, int BX2 = 0,
+          int CK = 8>
 FusedKernel make_group()
 {
-    using K = gnl::Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW, AX2, BX2>;
+    using K = gnl::Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW, AX2, BX2, CK>;
     FusedKernel k;
-    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV, EM, BY, NPW, AX2, BX2>;
+    k.fng = gnl::k_plane_group<AX, BX, AY, G, NW, NH, CHIV, EM, BY, NPW, AX2, BX2, CK>;
     k.chiv = CHIV;
     k.group = G;
     k.group_scratch = sizeof(cplx) * K::GROUP_SCRATCH_CPLX;
@@ -742,7 +743,8 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             cudaGetLastError();
             h->gk = FusedKernel();
         } else {
-            h->gk_grid = (sms / h->gk.group) * h->gk.group;
+            if (occ > 2) occ = 2;
+            h->gk_grid = ((sms * occ) / h->gk.group) * h->gk.group;
         }
     }
     if (ok && h->gk.fng && !h->fused) {

@@ -85,7 +85,9 @@ __device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uin
 // BY: radix of the second y stage (Ny = AY * BY; 8, or 16 for Ny = 384); NPW: row pairs per warp item (NPW * BY <= 32).
 // AX2 x BX2: the split of Nx used by the x-analysis (X2) when it differs from the synthesis' (768 = 48 x 16 on the way in,
 // 24 x 32 on the way back: every thread has an item in the stage that carries the pruned radix).
-template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_, int BY_ = 8, int NPW_ = 3, int AX2_ = 0, int BX2_ = 0>
+// CK: stored columns per column unit (8: 128 B runs in both hand-overs; 4: 64 B runs, for CTAs of 4 warps, two per SM).
+template <int AX_, int BX_, int AY_, int G_, int NW_, int NH_, bool CHIV_, int BY_ = 8, int NPW_ = 3, int AX2_ = 0, int BX2_ = 0,
+          int CK_ = 8>
 struct Grouped {
     static constexpr int AX2 = AX2_ ? AX2_ : AX_, BX2 = BX2_ ? BX2_ : BX_, C22 = BX2 / 2;
     static constexpr int BPX2 = Tile<AX2, BX2>::BP;
@@ -95,7 +97,7 @@ struct Grouped {
     static constexpr int NX = AX * BX, NY = BY * AY, C2 = BX / 2;
     static constexpr int NKY0 = NY / 3, W2 = 2 * NKY0, NPAIR = NX / 2;
     static constexpr int M = NX / 3, NX0 = 2 * M;
-    static constexpr int CK = 8;                       // stored columns per unit: 128 B runs in both hand-overs
+    static constexpr int CK = CK_;                     // stored columns per unit
     static constexpr int NUNIT = NKY0 / CK;            // column units per plane
     static constexpr int UPC = NUNIT / G_;             // column units per CTA
     static constexpr int PPG = NPAIR / G;              // row pairs per CTA
@@ -124,6 +126,7 @@ struct Grouped {
     static constexpr int NBAR = 1 + NW;                // mbarriers: column block, rows of each warp
     static constexpr int SMEM_CPLX = A_CPLX + TWX + TWX2 + TWY + (NBAR + 1) / 2;
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
+    static constexpr int MINB = (NW <= 4 && SMEM_BYTES <= 113 * 1024) ? 2 : 1;   // CTAs per SM the kernel is built for
     static constexpr size_t ZS_CPLX = (size_t)NPAIR * 2 * W2, PS_CPLX = (size_t)NPAIR * W2;   // per-group scratch
     static constexpr size_t GROUP_SCRATCH_CPLX = NF * ZS_CPLX + PS_CPLX;
     static_assert(AX % 3 == 0 && AY % 3 == 0 && AX % NH == 0 && BX % 2 == 0, "3/2 rule; k1 passes; row pairs");
@@ -139,15 +142,16 @@ struct Grouped {
 // EM (!CHIV only): chi = phi_bar - v_par A_par_bar composed in real space, by linearity: R holds the
 // real-space fields of phi_bar, R2 those of A_par_bar (one plane per (z, slab) each), vp[v + nv * species] the v_par
 // coefficients; slab sl of the launch is global slab slab0 + sl = w + nw * species.
-template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW_ = 3, int AX2_ = 0, int BX2_ = 0>
-__global__ void __launch_bounds__(32 * NW, 1)
+template <int AX, int BX, int AY, int G, int NW, int NH, bool CHIV, bool EM = false, int BY = 8, int NPW_ = 3, int AX2_ = 0, int BX2_ = 0,
+          int CK_ = 8>
+__global__ void __launch_bounds__(32 * NW, (Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW_, AX2_, BX2_, CK_>::MINB))
 k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __restrict__ R, const cplx* __restrict__ chi,
               const cplx* __restrict__ twx_g, const cplx* __restrict__ twy_g, cplx* __restrict__ scratch,
               unsigned* __restrict__ cnt, int nz, int nv, int nslab, double kxmin, double kymin, double coef,
               const cplx* __restrict__ R2 = nullptr, const double* __restrict__ vp = nullptr, int nw = 1, int slab0 = 0)
 {
     static_assert(!(EM && CHIV), "the composition needs chi-like fields shared over v");
-    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW_, AX2_, BX2_>;
+    using K = Grouped<AX, BX, AY, G, NW, NH, CHIV, BY, NPW_, AX2_, BX2_, CK_>;
     constexpr int BYP = K::BYP, AX2 = K::AX2, BX2 = K::BX2, C22 = K::C22, BPX2 = K::BPX2, AX21 = K::AX2 / 3;
     constexpr int NX = K::NX, NY = K::NY, C2 = K::C2, NKY0 = K::NKY0, W2 = K::W2, NPAIR = K::NPAIR, NF = K::NF;
     constexpr int M = K::M, NX0 = K::NX0, CK = K::CK, PPG = K::PPG, NPW = K::NPW, NT = K::NT, UPC = K::UPC, UPP = K::UPP;
