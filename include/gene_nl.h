@@ -141,6 +141,11 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
  *                           cluster's shared memory and distributed-shared-memory hand-overs (1.03 x the algorithmic
  *                           bytes; slower: DSMEM stores run at 18 B/clk/SM and 15 clusters fit the 148 SMs).  Same sizes.
  *   GENE_NL_KERNEL_BATCHED  the batched kernels (scratch through HBM/L2 in large batches) whatever the size.
+ *   GENE_NL_KERNEL_WARP     the group kernel with warp-autonomous x phases as well (a warp takes two adjacent columns
+ *                           through both x stages in its own shared-memory tile; every warp arrives on the hand-over
+ *                           counters; no CTA-wide barrier in the plane loop).  Measured on B200: 3 % faster than the
+ *                           group kernel at 384 x 192, 10 % slower at 768 x 384 and 144 x 144 (DESIGN.md sect. 6g), so
+ *                           it is an option, not the default.  Same sizes as the group kernel, not with GENE_NL_CHI_EM.
  * GENE_NL_EUNSUPPORTED when the plan has no such kernel.  Same results to rounding (all are checked against the
  * oracle).  Synchronises the device and re-allocates the scratch, like gene_nl_set_scratch_bytes.
  */
@@ -148,6 +153,7 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
 #define GENE_NL_KERNEL_CLUSTER 1
 #define GENE_NL_KERNEL_GROUP 2
 #define GENE_NL_KERNEL_BATCHED 3
+#define GENE_NL_KERNEL_WARP 4
 int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind);
 
 /*
@@ -156,7 +162,7 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind);
  *   5 algorithmic bytes per plane  B = 16*nx0*nky0*(3 + c),
  *   6 conventional flops per plane F = (3+2c)*T2D + 4M(1+c) + 3NxNy + 4M,
  *   with c = 1 if chi_has_v else 1/nv; 7: 1 if a fused (shared-memory resident) kernel is used, else 0;
- *   8: 1 if that kernel is the cluster kernel, 2 if it is the group kernel (gene_nl_set_plane_kernel), else 0.
+ *   8: 1 if that kernel is the cluster kernel, 2 the group kernel, 4 its warp-autonomous form (gene_nl_set_plane_kernel), else 0.
  *   Returns NaN for an unknown `what` or NULL plan.
  */
 double gene_nl_query(const gene_nl_plan* h, int what);

@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = (
     "gene_nlx_create", "gene_nlx_compute", "gene_nlx_compute_host", "gene_nlx_destroy", "gene_nlx_query",
 )
 # ... and include/gene_nl_bench.h (benchmark-only helpers, not on the hot path)
-BENCH_SYMBOLS = ("gene_nl_compute_profiled", "gene_nl_probe_peaks")
+BENCH_SYMBOLS = ("gene_nl_compute_profiled", "gene_nl_probe_peaks", "gene_nl_probe_exchange")
 
 _lock = threading.Lock()
 _lib = None
@@ -76,6 +76,8 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_query.restype = dbl
         lib.gene_nl_probe_peaks.argtypes = [ctypes.POINTER(dbl)]
         lib.gene_nl_probe_peaks.restype = i
+        lib.gene_nl_probe_exchange.argtypes = [ctypes.POINTER(dbl)]
+        lib.gene_nl_probe_exchange.restype = i
         ll = ctypes.c_longlong
         lib.gene_nlx_create.argtypes = [i, i, ll]
         lib.gene_nlx_create.restype = vp
@@ -157,7 +159,7 @@ def gene_nl_set_scratch_bytes(h, nbytes: int) -> None:
         raise GeneNLError(f"gene_nl_set_scratch_bytes failed ({rc}): {gene_nl_last_error()}")
 
 
-GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP, GENE_NL_KERNEL_BATCHED = 0, 1, 2, 3
+GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP, GENE_NL_KERNEL_BATCHED, GENE_NL_KERNEL_WARP = 0, 1, 2, 3, 4
 
 
 def gene_nl_set_plane_kernel(h, kind: int) -> None:
@@ -217,6 +219,16 @@ def gene_nl_probe_peaks():
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_probe_peaks failed ({rc})")
     return float(out[0]), float(out[1]), float(out[2])
+
+
+def gene_nl_probe_exchange():
+    """ns per iteration and 8 warps of (FP64 butterflies alone, + exchange through shared memory, + exchange by warp
+    shuffles) with 8 warps per SM, then the same three with 16 warps per SM."""
+    out = (ctypes.c_double * 6)()
+    rc = load_library().gene_nl_probe_exchange(out)
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_probe_exchange failed ({rc})")
+    return tuple(float(v) for v in out)
 
 
 # ---- x-global variant (include/gene_nl.h, gene_nlx_*) ----

@@ -21,6 +21,7 @@
 #include "nl_fused2.cuh"
 #include "nl_cluster.cuh"
 #include "nl_group.cuh"
+#include "nl_wa.cuh"
 #include "nl_kernels.cuh"
 #include "nl_pipe.cuh"
 
@@ -61,6 +62,7 @@ struct FusedKernel {
     cluster_fn fnc = nullptr; // the plane spread over a thread-block cluster (nl_cluster.cuh); chi shared over v only
     group_fn fng = nullptr;   // the plane spread over a group of co-resident CTAs, hand-overs through L2 (nl_group.cuh)
     bool chiv = false;        // group kernel: chi per plane goes through the kernel too (no chi-side launches)
+    bool wa = false;          // fng is the warp-autonomous form (nl_wa.cuh)
     int group = 1;            // CTAs per group
     size_t group_scratch = 0; // bytes of Z + P scratch per group
     int cluster = 1;          // CTAs per cluster
@@ -93,6 +95,32 @@ FusedKernel make_group()
     k.smem = K::SMEM_BYTES;
     k.nt = K::NT;
     return k;
+}
+
+template <int AX, int BX, int AY, int BY, int G, int NW, bool CHIV, bool EM, int NPW, bool PF, int AX2 = 0, int BX2 = 0>
+FusedKernel make_wa()
+{
+    using K = gnl::WarpAuto<AX, BX, AY, BY, G, NW, CHIV, NPW, AX2, BX2>;
+    FusedKernel k;
+    k.fng = gnl::k_plane_wa<AX, BX, AY, BY, G, NW, CHIV, EM, NPW, PF, AX2, BX2>;
+    k.wa = true;
+    k.chiv = CHIV;
+    k.group = G;
+    k.group_scratch = sizeof(cplx) * K::GROUP_SCRATCH_CPLX;
+    k.smem = K::SMEM_BYTES;
+    k.nt = K::NT;
+    return k;
+}
+
+// The warp-autonomous form of the group kernel (nl_wa.cuh): same groups and scratch, no CTA-wide barrier in the plane loop
+bool find_wa(int nx, int ny, bool chi_has_v, bool em, FusedKernel* out)
+{
+    if (em) return false;   // (the composition of chi on the device stays with the group kernel)
+    if (nx == 384 && ny == 192 && !chi_has_v) { *out = make_wa<24, 16, 24, 8, 4, 8, false, false, 3, true>(); return out->smem <= 227 * 1024; }
+    if (nx == 768 && ny == 384 && !chi_has_v) { *out = make_wa<24, 32, 24, 16, 8, 8, false, false, 2, false>(); return out->smem <= 227 * 1024; }
+    if (nx == 144 && ny == 144 && chi_has_v) { *out = make_wa<12, 12, 18, 8, 1, 8, true, false, 3, true>(); return out->smem <= 227 * 1024; }
+    if (nx == 144 && ny == 144 && !chi_has_v) { *out = make_wa<12, 12, 18, 8, 1, 8, false, false, 3, true>(); return out->smem <= 227 * 1024; }
+    return false;
 }
 
 // Planes beyond one SM: groups of G co-resident CTAs per plane, Z and P through L2
@@ -323,6 +351,8 @@ struct gene_nl_plan {
     FusedKernel fk;
     FusedKernel gk;           // the group kernel for this plane size, if there is one
     int gk_grid = 0;          // its grid: co-resident groups x CTAs per group
+    FusedKernel wk;           // the warp-autonomous group kernel for this plane size, if there is one
+    int wk_grid = 0;
     FusedKernel ck;           // the cluster kernel for this plane size, if there is one (gene_nl_set_plane_kernel)
     int ck_grid = 0;          // its grid: resident clusters x CTAs per cluster
     FusedKernel fk_auto;      // what gene_nl_create selected
@@ -698,6 +728,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     // replaced DSMEM by an L2-resident scratch and clusters by groups of a cooperative launch: see below.
     if (!h->fused && !h->em && !h->chi_has_v) find_cluster(h->Nx, h->Ny, &h->ck);
     if (!h->fused) find_group(h->Nx, h->Ny, h->chi_has_v != 0, h->em, &h->gk);
+    if (!h->fused) find_wa(h->Nx, h->Ny, h->chi_has_v != 0, h->em, &h->wk);
     if (h->fused) {
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -712,6 +743,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
               set_smem(h->yk.br, h->yk.smem_br, "k_ybracket smem") && set_smem(h->yk.real, h->yk.smem_real, "k_yreal smem") &&
               (!h->ck.fnc || set_smem(h->ck.fnc, h->ck.smem, "k_plane_cluster smem")) &&
               (!h->gk.fng || set_smem(h->gk.fng, h->gk.smem, "k_plane_group smem")) &&
+              (!h->wk.fng || set_smem(h->wk.fng, h->wk.smem, "k_plane_wa smem")) &&
               (!h->fused || (h->fk.fn2 ? set_smem(h->fk.fn2, h->fk.smem, "k_plane_fused2 smem")
                                        : set_smem(h->fk.fn, h->fk.smem, "k_plane_fused smem"))) &&
               upload_const_twiddles();
@@ -745,6 +777,18 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
         } else {
             if (occ > 2) occ = 2;
             h->gk_grid = ((sms * occ) / h->gk.group) * h->gk.group;
+        }
+    }
+    if (ok && h->wk.fng) {  // co-resident groups (cooperative launch), one CTA per SM
+        int sms = 0, occ = 0, coop = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (!coop || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->wk.fng, h->wk.nt, h->wk.smem) != cudaSuccess || occ < 1 ||
+            sms < h->wk.group) {
+            cudaGetLastError();
+            h->wk = FusedKernel();
+        } else {
+            h->wk_grid = (sms / h->wk.group) * h->wk.group;
         }
     }
     if (ok && h->gk.fng && !h->fused) {
@@ -860,12 +904,17 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
 {
     g_err.clear();
     if (!h) { set_err("NULL plan"); return GENE_NL_EINVAL; }
-    if (kind != GENE_NL_KERNEL_AUTO && kind != GENE_NL_KERNEL_CLUSTER && kind != GENE_NL_KERNEL_GROUP && kind != GENE_NL_KERNEL_BATCHED) {
+    if (kind != GENE_NL_KERNEL_AUTO && kind != GENE_NL_KERNEL_CLUSTER && kind != GENE_NL_KERNEL_GROUP && kind != GENE_NL_KERNEL_BATCHED &&
+        kind != GENE_NL_KERNEL_WARP) {
         set_err("gene_nl_set_plane_kernel: unknown kind");
         return GENE_NL_EINVAL;
     }
     if (kind == GENE_NL_KERNEL_GROUP && !h->gk.fng) {
         set_err("gene_nl_set_plane_kernel: no group kernel for this plan (384 x 192 padded grid, chi shared over v, cooperative launch)");
+        return GENE_NL_EUNSUPPORTED;
+    }
+    if (kind == GENE_NL_KERNEL_WARP && !h->wk.fng) {
+        set_err("gene_nl_set_plane_kernel: no warp-autonomous group kernel for this plan (384 x 192 or 768 x 384 with chi shared over v, 144 x 144; not with GENE_NL_CHI_EM)");
         return GENE_NL_EUNSUPPORTED;
     }
     if (kind == GENE_NL_KERNEL_CLUSTER && !h->ck.fnc) {
@@ -878,6 +927,7 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
     free_scratch(&h->scr);
     if (kind == GENE_NL_KERNEL_CLUSTER) { h->fk = h->ck; h->fused = true; h->fused_grid = h->ck_grid; }
     else if (kind == GENE_NL_KERNEL_GROUP) { h->fk = h->gk; h->fused = true; h->fused_grid = h->gk_grid; }
+    else if (kind == GENE_NL_KERNEL_WARP) { h->fk = h->wk; h->fused = true; h->fused_grid = h->wk_grid; }
     else if (kind == GENE_NL_KERNEL_BATCHED) { h->fk = FusedKernel(); h->fused = false; h->fused_grid = 0; }
     else { h->fk = h->fk_auto; h->fused = h->fused_auto; h->fused_grid = h->fused_grid_auto; }
     configure_batching(h);
@@ -1103,7 +1153,7 @@ double gene_nl_query(const gene_nl_plan* h, int what)
     case 4: return h->fused ? (double)((h->nw * h->nspec + h->nss - 1) / h->nss)
                             : (double)h->nw * h->nspec * chunks_per_slab(h) * ((h->nv + h->nvb - 1) / h->nvb);
     case 7: return h->fused ? 1.0 : 0.0;
-    case 8: return h->fk.fnc ? 1.0 : (h->fk.fng ? 2.0 : 0.0);
+    case 8: return h->fk.fnc ? 1.0 : (h->fk.fng ? (h->fk.wa ? 4.0 : 2.0) : 0.0);
     case 5: return 16.0 * M * (3.0 + c);
     case 6: {
         const double t2d = h->nky0 * 5.0 * Nx * std::log2(Nx) + Nx * 2.5 * Ny * std::log2(Ny);

@@ -196,7 +196,7 @@ SPREAD_SHAPES = [(256, 64, 1, 1, 1, 1),       # one plane: one cluster / group b
                  (256, 64, 2, 3, 1, 1),
                  (256, 64, 3, 5, 2, 2),       # 60 planes: several planes per cluster / group, chi shared by 5 planes
                  (256, 64, 36, 2, 1, 1)]
-SPREAD_KINDS = [1, 2, 3]                      # GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP (the default here), GENE_NL_KERNEL_BATCHED
+SPREAD_KINDS = [1, 2, 3, 4]                   # GENE_NL_KERNEL_CLUSTER, _GROUP (the default here), _BATCHED, _WARP
 
 
 @pytest.mark.parametrize("kind", SPREAD_KINDS)
@@ -205,7 +205,7 @@ def test_spread_kernels_small_shapes_all_planes(cuda_device, nx0, nky0, nz, nv, 
     from paper_1310_1485_b200 import GeneNL
     wl = W.small_workload(nx0, nky0, nz, nv, nw, nspec, 0.03, 0.07, False, seed=300 + nz + nv)
     with GeneNL(wl, plane_kernel=kind) as nl:
-        assert (nl.query(7), nl.query(8)) == ((1.0, float(kind)) if kind < 3 else (0.0, 0.0))   # the requested kernel runs
+        assert (nl.query(7), nl.query(8)) == ((1.0, float(kind)) if kind != 3 else (0.0, 0.0))   # the requested kernel runs
     with GeneNL(wl) as nl:
         assert nl.query(8) == 2.0                                   # and the group kernel is the default at this size
     check_parity(wl, cuda_device, plane_kernel=kind)
@@ -263,7 +263,7 @@ def test_spread_kernels_properties_and_selection(cuda_device, kind):
 
 # 144 x 144 planes (the shape of configs[4]): the group kernel with chi per plane (chi goes through the kernel like g) and
 # with chi shared over v, and the batched kernels on the same data
-@pytest.mark.parametrize("kind", [2, 3])
+@pytest.mark.parametrize("kind", [2, 3, 4])
 @pytest.mark.parametrize("chi_has_v", [True, False])
 @pytest.mark.parametrize("nz,nv,nw,nspec", [(1, 1, 1, 1), (3, 5, 2, 2), (37, 2, 1, 1)])
 def test_group_kernel_144x144_planes(cuda_device, nz, nv, nw, nspec, chi_has_v, kind):
@@ -288,6 +288,9 @@ def test_group_kernel_144x144_planes(cuda_device, nz, nv, nw, nspec, chi_has_v, 
     (96, 48, True, 2),           # k_plane_group with chi per plane (groups of one CTA)
     (512, 128, False, 2),        # k_plane_group, radix-16 second y stage
     (256, 64, True, 3),          # batched kernels
+    (256, 64, False, 4),         # k_plane_wa: per-warp tiles, every warp on the hand-over counters
+    (96, 48, True, 4),           # k_plane_wa with chi per plane
+    (512, 128, False, 4),        # k_plane_wa, radix-32 x stages
 ])
 def test_repeated_runs_give_the_same_bits(cuda_device, nx0, nky0, chi_has_v, kind):
     """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so a data race in the shared-memory /
