@@ -518,6 +518,9 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
     flops = per_kernel_flops(my, fused=nl.query(7) == 1.0)
     if my.chi_has_v and not prof_n.get("k_yreal") and "k_yreal" in flops and "k_ybracket" in flops:
         flops["k_ybracket"] += flops.pop("k_yreal")  # chi's y-synthesis runs inside k_ybracket_cv (no k_yreal launches)
+    if "k_plane_fused" in flops and not prof_n.get("k_xinv") and not prof_n.get("k_yreal"):
+        # chi per plane goes through the plane kernel itself (group kernel, CHIV): its transforms are that kernel's work
+        flops["k_plane_fused"] += flops.pop("k_xinv", 0.0) + flops.pop("k_yreal", 0.0)
     fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
     if "probe" not in env:
         try:
@@ -539,8 +542,9 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
     traffic = cap[dom][0] if dom in cap else None
     traffic_step = None
     if cap and all(k in cap for k in kernels):
-        # whole step: every kernel's bytes per plane of its launch x the planes (chi planes for the chi-side kernels)
-        traffic_step = sum(cap[k][0] / cap[k][1] * (my.chi_planes if k == "k_yreal" else my.planes) for k in kernels)
+        # whole step: every kernel class's captured bytes per launch (average over the launches of one step of the full
+        # workload) x the launches this run made per step
+        traffic_step = sum(cap[k][0] * kernels[k]["launches_per_step"] for k in kernels)
     roofline = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
                 "unit": "TFLOP/s", "frac": kernels[dom]["tflops"] / fp64_model, "traffic": traffic,
                 "traffic_note": why or ("ncu --set full capture stamped with src_sha16 %s" % source_sha16()),

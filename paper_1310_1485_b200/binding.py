@@ -223,8 +223,8 @@ def gene_nl_probe_peaks():
 
 def gene_nl_probe_exchange():
     """ns per iteration and 8 warps of (FP64 butterflies alone, + exchange through shared memory, + exchange by warp
-    shuffles) with 8 warps per SM, then the same three with 16 warps per SM."""
-    out = (ctypes.c_double * 6)()
+    shuffles) with 8 warps per SM, the same three with 16 warps per SM, and with 8 warps and twice the FP64 work."""
+    out = (ctypes.c_double * 9)()
     rc = load_library().gene_nl_probe_exchange(out)
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_probe_exchange failed ({rc})")

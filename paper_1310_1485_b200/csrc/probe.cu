@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(256) k_probe_smem(double* out, int iters)
 // FP64 work of about one radix-8 butterfly per 8 values ("Warp shuffles of FP64 data are 2x32-bit shuffles
 // per double ... measure before relying on warp-shuffle butterflies").  MODE 0: the FMAs alone; 1: + exchange through a
 // per-warp shared-memory tile (8 x STS.128, 8 x LDS.128, conflict free); 2: + exchange by shuffles (8 x 4 SHFL.BFLY).
-template <int MODE>
+template <int MODE, int U>
 __global__ void __launch_bounds__(256) k_probe_xchg(double* out, int iters, double b, double c)
 {
     extern __shared__ double2 buf[];
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(256) k_probe_xchg(double* out, int iters, doub
     for (int j = 0; j < 8; ++j) v[j] = make_double2(1.0 + 1e-3 * (lane + 32 * j), 0.5 - 1e-3 * j);
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-        for (int u = 0; u < 5; ++u) {   // 80 FP64 instructions per 8 values (a twiddled radix 8 has 76)
+        for (int u = 0; u < U; ++u) {   // U = 5: 80 FP64 instructions per 8 values (a twiddled radix 8 has 76)
 #pragma unroll
             for (int j = 0; j < 8; ++j) {
                 v[j].x = fma(v[j].x, b, c);
@@ -93,9 +93,9 @@ __global__ void __launch_bounds__(256) k_probe_xchg(double* out, int iters, doub
 
 }  // namespace
 
-extern "C" int gene_nl_probe_exchange(double* out6)
+extern "C" int gene_nl_probe_exchange(double* out9)
 {
-    if (!out6) return GENE_NL_EINVAL;
+    if (!out9) return GENE_NL_EINVAL;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return GENE_NL_ECUDA;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
@@ -106,21 +106,28 @@ extern "C" int gene_nl_probe_exchange(double* out6)
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
-    for (int occ = 1; occ <= 2; ++occ)
+    for (int cfg = 0; cfg < 3; ++cfg)   // 8 warps per SM; 16 warps per SM; 8 warps per SM with twice the FP64 work
     for (int mode = 0; mode < 3; ++mode) {
+        const int occ = cfg == 1 ? 2 : 1;
         const int blocks = occ * sms;
         float best = 1e30f, ms = 0.f;
         for (int rep = 0; rep < 4; ++rep) {
             cudaEventRecord(e0);
-            if (mode == 0) k_probe_xchg<0><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-            else if (mode == 1) k_probe_xchg<1><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-            else k_probe_xchg<2><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+            if (cfg < 2) {
+                if (mode == 0) k_probe_xchg<0, 5><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+                else if (mode == 1) k_probe_xchg<1, 5><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+                else k_probe_xchg<2, 5><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+            } else {
+                if (mode == 0) k_probe_xchg<0, 10><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+                else if (mode == 1) k_probe_xchg<1, 10><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+                else k_probe_xchg<2, 10><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
+            }
             cudaEventRecord(e1);
             cudaEventSynchronize(e1);
             cudaEventElapsedTime(&ms, e0, e1);
             if (rep > 0 && ms < best) best = ms;
         }
-        out6[3 * (occ - 1) + mode] = (double)best * 1e6 / iters / occ;   // ns per iteration (8 values per lane) and 8 warps of an SM
+        out9[3 * cfg + mode] = (double)best * 1e6 / iters / occ;   // ns per iteration (8 values per lane) and 8 warps of an SM
     }
     cudaError_t err = cudaDeviceSynchronize();
     cudaEventDestroy(e0);
