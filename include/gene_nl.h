@@ -49,8 +49,8 @@ typedef struct gene_nl_plan gene_nl_plan; /* opaque */
 
 /*
  * gene_nl_create -- build a plan on the CURRENT CUDA device (north_star signature).
- *   nx0   number of kx modes (even; Nx = 3*nx0/2 must be one of 24,48,96,144,192,384,768)
- *   nky0  number of ky >= 0 modes (Ny = 3*nky0 must be one of 24,48,96,144,192,384)
+ *   nx0   number of kx modes (even; Nx = 3*nx0/2 must be one of 24,48,96,144,192,288,384,576,768,1152,1536)
+ *   nky0  number of ky >= 0 modes (Ny = 3*nky0 must be one of 24,48,96,144,192,288,384,576)
  *   nz, nv, nw, nspec   extents of the parametric dimensions (all > 0); planes = nz*nv*nw*nspec
  *   kxmin, kymin        wavenumber spacings (finite)
  *   chi_has_v           0: chi has no v extent (shared by the nv planes); 1: chi shaped like g

@@ -270,7 +270,11 @@ bool find_x(int nx, XKernels* out)
     case 96: *out = make_x<96, 12, 8, 8, 128>(); return true;
     case 144: *out = make_x<144, 12, 12, 8, 128>(); return true;
     case 192: *out = make_x<192, 24, 8, 8, 128>(); return true;
+    case 288: *out = make_x<288, 18, 16, 4, 128>(); return true;
     case 384: *out = make_x<384, 24, 16, 4, 128>(); return true;
+    case 576: *out = make_x<576, 24, 24, 4, 128>(); return true;
+    case 1152: *out = make_x<1152, 36, 32, 4, 128>(); return true;
+    case 1536: *out = make_x<1536, 48, 32, 2, 128>(); return true;
     case 768: *out = make_x<768, 24, 32, 4, 128>();
         // row-major Z in 128 B pieces: 8 columns per CTA, the two signs one after the other through the same 8 tiles
         // of E (measured on B200, configs[3]: k_xinv 36.0 -> 32.7 ms)
@@ -290,7 +294,9 @@ bool find_y(int ny, int nx, YKernels* out)
     case 96: *out = rp8 ? make_y<96, 12, 8, 8, 64>() : make_y<96, 12, 8, 4, 64>(); return true;
     case 144: *out = rp8 ? make_y<144, 12, 12, 8, 96>() : make_y<144, 12, 12, 4, 96>(); return true;
     case 192: *out = make_y<192, 12, 16, 4, 64>(); return true;
+    case 288: *out = make_y<288, 18, 16, 4, 64>(); return true;
     case 384: *out = make_y<384, 24, 16, 4, 64>(); return true;
+    case 576: *out = make_y<576, 24, 24, 4, 96>(); return true;
     default: return false;
     }
 }
@@ -707,8 +713,8 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
     h->planes = (long long)nz * nv * nw * nspec;
     h->device = dev;
     if (!find_x(h->Nx, &h->xk) || !find_y(h->Ny, h->Nx, &h->yk)) {
-        char buf[160];
-        snprintf(buf, sizeof buf, "gene_nl_create: unsupported padded grid %dx%d (Nx in {24,48,96,144,192,384,768}, Ny in {24,48,96,144,192,384})", h->Nx, h->Ny);
+        char buf[256];
+        snprintf(buf, sizeof buf, "gene_nl_create: unsupported padded grid %dx%d (Nx in {24,48,96,144,192,288,384,576,768,1152,1536}, Ny in {24,48,96,144,192,288,384,576})", h->Nx, h->Ny);
         set_err(buf);
         delete h;
         return nullptr;

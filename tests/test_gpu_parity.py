@@ -40,6 +40,11 @@ SHAPES = [
     (512, 16, 2, 3, 1, 1, False), (512, 64, 1, 2, 1, 1, False),
     (512, 128, 1, 2, 1, 1, False),   # the plane shape of configs[3]: k_xinv<768,...,SEQ> + k_ybracket<384> + k_xfwd<768>
     (512, 128, 1, 1, 1, 1, True),
+    # the wider size list (2^a 3^b): Nx = 288, 576, 1152, 1536 and Ny = 288, 576 (batched kernels)
+    (192, 32, 2, 3, 1, 1, False), (192, 96, 1, 2, 1, 1, True),     # 288 x 96 (transposed-Z path), 288 x 288
+    (384, 96, 1, 2, 1, 1, False), (32, 192, 2, 2, 1, 1, False),    # 576 x 288, 48 x 576
+    (768, 16, 1, 2, 1, 1, True), (1024, 16, 1, 3, 1, 1, False),    # 1152 x 48, 1536 x 48
+    (1024, 64, 1, 1, 1, 1, False),                                 # 1536 x 192: 64 Ki modes per plane
 ]
 
 
