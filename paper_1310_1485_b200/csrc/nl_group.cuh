@@ -293,13 +293,16 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 __syncthreads();  // E is free for the next k1 pass / the next step
             }
         }
-        // ---- hand-over 1: every CTA of the group has written its columns of Z ----
-        if (tid == 0) {
-            __threadfence();
-            atomicAdd(zcnt, 1u);
-            while (ld_acquire_gpu(zcnt) < (unsigned)G * (it + 1)) {}
+        // ---- hand-over 1: every CTA of the group has written its columns of Z (a group of one: the CTA barrier that
+        // ended X1 has ordered the stores; no counter) ----
+        if constexpr (G > 1) {
+            if (tid == 0) {
+                __threadfence();
+                atomicAdd(zcnt, 1u);
+                while (ld_acquire_gpu(zcnt) < (unsigned)G * (it + 1)) {}
+            }
+            __syncthreads();
         }
-        __syncthreads();
 
         // =============== Y: this CTA's row pairs, a warp takes NPW of them at a time, __syncwarp only ===============
         {
@@ -502,12 +505,14 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
         }
         // ---- hand-over 2: every CTA of the group has written its rows of P ----
         __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            atomicAdd(pcnt, 1u);
-            while (ld_acquire_gpu(pcnt) < (unsigned)G * (it + 1)) {}
+        if constexpr (G > 1) {
+            if (tid == 0) {
+                __threadfence();
+                atomicAdd(pcnt, 1u);
+                while (ld_acquire_gpu(pcnt) < (unsigned)G * (it + 1)) {}
+            }
+            __syncthreads();
         }
-        __syncthreads();
 
         // =============== X2: x-analysis of this CTA's column units, UPP at a time; delete modes, prefactor, add ===============
         if (tid == 0 && t + (unsigned)ngroup < T) request_block(t + (unsigned)ngroup, 0);   // lands behind the x tiles
