@@ -261,7 +261,7 @@ def xglobal_main(args):
     traffic = cap["k_xglobal"][0] * wl.planes / cap["k_xglobal"][1] if "k_xglobal" in cap else None
     roofline = {"kernel": "k_xglobal", "bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
                 "frac": gbs / hbm_peak, "traffic": traffic,
-                "traffic_note": why or ("ncu --set full capture stamped with src_sha16 %s" % source_sha16()),
+                "traffic_note": why or ("ncu dram__bytes capture of one whole step (profiles/r02_dram.md), stamped with src_sha16 %s" % source_sha16()),
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
                 "bytes_per_plane": B, "flops_per_plane": F, "achieved_tflops": F * wl.planes / (ms_per_step * 1e-3) / 1e12,
                 "share_of_step": 1.0}
@@ -547,7 +547,7 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
         traffic_step = sum(cap[k][0] * kernels[k]["launches_per_step"] for k in kernels)
     roofline = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
                 "unit": "TFLOP/s", "frac": kernels[dom]["tflops"] / fp64_model, "traffic": traffic,
-                "traffic_note": why or ("ncu --set full capture stamped with src_sha16 %s" % source_sha16()),
+                "traffic_note": why or ("ncu dram__bytes capture of one whole step (profiles/r02_dram.md), stamped with src_sha16 %s" % source_sha16()),
                 "peak_source": "model 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md sect. 7)",
                 "peak_measured_dfma": probe_tf, "smem_gbs_measured": probe_smem_gbs,
                 "share_of_step": kernels[dom]["ms_per_step"] / sum(v["ms_per_step"] for v in kernels.values())}
