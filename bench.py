@@ -283,10 +283,30 @@ def xglobal_main(args):
             once()
         barrier()
         dt = time.perf_counter() - t0
+        # the paper's own roofline for this path, redrawn: what the host link alone allows.  Measured
+        # here with plain pinned copies of one array (CUDA events), not taken from a data sheet.
+        def link_gbs(dst, src):
+            ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            dst.copy_(src, non_blocking=True)
+            torch.cuda.synchronize()
+            ev0.record()
+            for _ in range(3):
+                dst.copy_(src, non_blocking=True)
+            ev1.record()
+            torch.cuda.synchronize()
+            return 3 * src.numel() * src.element_size() / (ev0.elapsed_time(ev1) * 1e-3) / 1e9
+        dev_buf = torch.empty_like(host[0], device=dev)
+        h2d, d2h = link_gbs(dev_buf, host[0]), link_gbs(host[0].clone().pin_memory(), dev_buf)
+        del dev_buf
+        U = wl.plane_bytes
         e2e = {"value": n * world * args.e2e_steps / dt, "unit": UNIT, "h2d_bytes_per_step": 5 * n * wl.plane_bytes,
                "d2h_bytes_per_step": n * wl.plane_bytes, "steps": args.e2e_steps,
                "api": f"gene_nlx_compute_host on {n} planes (pinned host buffers, chunked over three streams)",
-               "link_roofline_planes_per_s": None}
+               "link_h2d_gbs": h2d, "link_d2h_gbs": d2h,
+               # full duplex: 5 planes in and 1 plane out per plane computed move at the same time
+               "link_roofline_planes_per_s": world / max(5 * U / (h2d * 1e9), U / (d2h * 1e9)),
+               # the paper's model: BW0 / 6 (transferable planes per second times the intensity 1/6, half duplex)
+               "paper_model_planes_per_s": world * h2d * 1e9 / (6 * U)}
         gene_nlx_destroy(h2)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
