@@ -183,7 +183,8 @@ double gene_nl_query(const gene_nl_plan* h, int what);
  * offset(x,j,p) = x + nx*(j + nky0*p); x is a real-space point, j the ky index (ky >= 0; ky < 0 implied by
  * reality; Im of the j = 0 entries is ignored).  pref: nx doubles (the x-dependent prefactor).
  * All pointers are DEVICE pointers, caller-owned, 16-byte aligned (pref: 8); rhs must not overlap an input.
- * Supported: nky0 in {8, 16, 32} (Ny = 24, 48, 96); any nx >= 1 (tiles of 16 x points, ragged tail allowed).
+ * Supported: nky0 in {8, 16, 32, 48, 64, 96, 128} (Ny = 24 .. 384); any nx >= 1 (tiles of 16 x points, 8 from
+ * nky0 = 48 on; ragged tail allowed).
  * Asynchronous on `stream`; one kernel launch per compute.  Errors as for gene_nl_* (gene_nl_last_error).
  * gene_nlx_compute_host takes HOST pointers (same layouts; pref a host array of nx doubles) and streams the planes
  * through the device in chunks on three CUDA streams ("we split each input array into (usually four)

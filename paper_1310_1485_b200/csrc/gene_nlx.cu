@@ -42,6 +42,11 @@ bool find_xg(int ny, XgKernel* out)
     case 24: *out = make_xg<24, 3, 8, 64, 16>(); return true;
     case 48: *out = make_xg<48, 6, 8, 64, 16>(); return true;   // the paper's 64 x 16 planes
     case 96: *out = make_xg<96, 12, 8, 64, 16>(); return true;
+    // longer y grids (not the paper's size): 8 x points per tile so that the staging and exchange tiles fit beside each other
+    case 144: *out = make_xg<144, 18, 8, 64, 8>(); return true;
+    case 192: *out = make_xg<192, 24, 8, 64, 8>(); return true;
+    case 288: *out = make_xg<288, 18, 16, 64, 8>(); return true;
+    case 384: *out = make_xg<384, 24, 16, 64, 8>(); return true;
     default: return false;
     }
 }
@@ -86,7 +91,7 @@ gene_nlx_plan* gene_nlx_create(int nx, int nky0, long long planes)
     gene_nlx_plan* h = new gene_nlx_plan();
     h->nx = nx; h->nky0 = nky0; h->Ny = 3 * nky0; h->planes = planes; h->device = dev;
     if (!find_xg(h->Ny, &h->k)) {
-        gene_nl_set_error_("gene_nlx_create: unsupported nky0 (padded y grid Ny = 3 nky0 must be 24, 48 or 96)");
+        gene_nl_set_error_("gene_nlx_create: unsupported nky0 (padded y grid Ny = 3 nky0 must be 24, 48, 96, 144, 192, 288 or 384)");
         delete h;
         return nullptr;
     }

@@ -38,7 +38,7 @@ def plane_errors(wl, arrs, out, planes):
 
 # every instantiated y length, x extents with a ragged tail (not a multiple of the 32-point tile), one plane
 @pytest.mark.parametrize("nx,nky0,planes", [(64, 16, 37), (32, 8, 5), (96, 32, 9), (40, 16, 7), (7, 8, 3), (1, 16, 1),
-                                            (33, 32, 2)])
+                                            (33, 32, 2), (24, 48, 3), (20, 64, 2), (16, 96, 2), (9, 128, 2)])
 def test_small_shapes_all_planes(cuda_device, nx, nky0, planes):
     wl = W.XGlobalWorkload(f"xg_{nx}x{nky0}", nx, nky0, planes, 100 + nx + nky0, 0.7)
     arrs = W.make_xglobal_inputs(wl, cuda_device)
