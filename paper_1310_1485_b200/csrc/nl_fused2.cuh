@@ -134,11 +134,9 @@ k_plane_fused2(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* _
             const long long tn = t + gridDim.x;
             if (tn < T) {
                 const size_t pn = plane_of(tn);
-                const char* a = (const char*)(g + pn * plane_elems);
-                const char* b = (const char*)(rhs + pn * plane_elems);
-                for (size_t off = (size_t)threadIdx.x * 128; off < plane_elems * sizeof(cplx); off += (size_t)NW * 32 * 128) {
-                    prefetch_l2(a + off);
-                    prefetch_l2(b + off);
+                if (threadIdx.x == 0) {   // one bulk prefetch per array (TMA, SASS UBLKPF) instead of a line-by-line loop (-0.5 %)
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(g + pn * plane_elems), "r"((uint32_t)(plane_elems * sizeof(cplx))) : "memory");
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rhs + pn * plane_elems), "r"((uint32_t)(plane_elems * sizeof(cplx))) : "memory");
                 }
             }
         }

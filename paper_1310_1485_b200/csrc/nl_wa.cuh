@@ -3,7 +3,7 @@
 // with no CTA-wide barrier left in the plane loop.
 //
 // Same steps and the same scratch layout as nl_group.cuh.  What the ncu capture of
-// that kernel showed (profiles/r02_ncu_group_summary.md): its y phase -- warps that run whole row pairs with
+// that kernel showed (profiles/r02_ncu_summary.md): its y phase -- warps that run whole row pairs with
 // __syncwarp only -- issues 54 % of the instructions in 36 % of the time, while the two x phases, whose 8 warps move
 // in lockstep through stage 1 / __syncthreads / stage 2 / __syncthreads, need 60 % of the time for the rest: in
 // lockstep all warps load, then all compute, then all store, so the FP64 pipe idles while the shared-memory pipe works
