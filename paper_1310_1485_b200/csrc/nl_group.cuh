@@ -370,9 +370,10 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 mbar_wait(ybar, yph);
                 yph ^= 1;
                 // The rows are in shared memory: their lines in the scratch are dead.  Dropping them pays where the groups'
-                // scratch exceeds what L2 keeps (768 x 384: 81 MB; DRAM writes 69 -> 34 GB per launch, time unchanged);
-                // at 384 x 192 (44 MB, already 1.07 x the algorithmic bytes) it cost 14 % of the time: not done there.
-                if constexpr (K::GROUP_SCRATCH_CPLX * sizeof(cplx) > ((size_t)2 << 20)) {
+                // scratch exceeds what L2 keeps (768 x 384: 85 MB; DRAM writes 69 -> 34 GB per launch, time unchanged;
+                // 144 x 144 with 148 groups of one CTA: 82 MB; DRAM traffic 2.0 -> 1.05 x the algorithmic bytes for 2 % of
+                // the time); at 384 x 192 (44 MB, already 1.05 x) it cost 14 % of the time: not done there.
+                if (K::GROUP_SCRATCH_CPLX * sizeof(cplx) * (size_t)ngroup > ((size_t)64 << 20)) {
                     constexpr int LPB = (int)(2 * W2 * sizeof(cplx) / 128);   // lines per pair block
                     for (int i = lane; i < NF * NPW * LPB; i += 32) {
                         const int j = i / LPB;
@@ -542,6 +543,12 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     for (int k2 = 0; k2 < BX2; ++k2) {
                         const cplx w = twx2[n1 * BPX2 + k2];
                         Ec[k2] = (k2 == 0) ? x[0] : cmul(x[k2], w.x, -w.y);
+                    }
+                    // the +ky halves of these P rows (one 128-byte line per row and unit, read by this warp instruction only)
+                    // are dead: drop them from L2 where the groups' scratch exceeds what L2 keeps
+                    if (K::GROUP_SCRATCH_CPLX * sizeof(cplx) * (size_t)ngroup > ((size_t)64 << 20) && col == 0 && CK == 8) {
+#pragma unroll
+                        for (int i = 0; i < C22; ++i) l2_discard_line(Ps + (size_t)(n1 + AX2 * i) * W2 + kyi);
                     }
                 }
                 cplx* Rcol = Rb + (size_t)((rank + G * (ub + us)) * CK + cols) * NX0 + k2s;
