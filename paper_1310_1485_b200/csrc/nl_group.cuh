@@ -130,6 +130,9 @@ struct Grouped {
     static constexpr int MINB = (NW <= 4 && SMEM_BYTES <= 113 * 1024) ? 2 : 1;   // CTAs per SM the kernel is built for
     static constexpr size_t ZS_CPLX = (size_t)NPAIR * 2 * W2, PS_CPLX = (size_t)NPAIR * W2;   // per-group scratch
     static constexpr size_t GROUP_SCRATCH_CPLX = NF * ZS_CPLX + PS_CPLX;
+    // consumed scratch lines are dropped from L2 where the scratch of all groups (148 SMs) exceeds what L2 keeps; a
+    // compile-time choice: at 384 x 192 the mere presence of the code costs 5 % (what ptxas hoists changes)
+    static constexpr bool DISCARD = GROUP_SCRATCH_CPLX * sizeof(cplx) * (148 / G_) > ((size_t)64 << 20);
     static_assert(AX % 3 == 0 && AY % 3 == 0 && AX % NH == 0 && BX % 2 == 0, "3/2 rule; k1 passes; row pairs");
     static_assert(NKY0 % CK == 0 && NUNIT % G == 0 && NPAIR % G == 0 && PPG % NPW == 0, "the group divides the work");
     static_assert(NPW * BY <= 32 && AY <= 32 && NKY0 == BY * (AY / 3) && (BY == 8 || BY == 16), "lanes of the y stages");
@@ -373,7 +376,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                 // scratch exceeds what L2 keeps (768 x 384: 85 MB; DRAM writes 69 -> 34 GB per launch, time unchanged;
                 // 144 x 144 with 148 groups of one CTA: 82 MB; DRAM traffic 2.0 -> 1.05 x the algorithmic bytes for 2 % of
                 // the time); at 384 x 192 (44 MB, already 1.05 x) it cost 14 % of the time: not done there.
-                if (K::GROUP_SCRATCH_CPLX * sizeof(cplx) * (size_t)ngroup > ((size_t)64 << 20)) {
+                if constexpr (K::DISCARD) {
                     constexpr int LPB = (int)(2 * W2 * sizeof(cplx) / 128);   // lines per pair block
                     for (int i = lane; i < NF * NPW * LPB; i += 32) {
                         const int j = i / LPB;
@@ -546,7 +549,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     }
                     // the +ky halves of these P rows (one 128-byte line per row and unit, read by this warp instruction only)
                     // are dead: drop them from L2 where the groups' scratch exceeds what L2 keeps
-                    if (K::GROUP_SCRATCH_CPLX * sizeof(cplx) * (size_t)ngroup > ((size_t)64 << 20) && col == 0 && CK == 8) {
+                    if (K::DISCARD && CK == 8 && col == 0) {
 #pragma unroll
                         for (int i = 0; i < C22; ++i) l2_discard_line(Ps + (size_t)(n1 + AX2 * i) * W2 + kyi);
                     }
