@@ -35,3 +35,26 @@ def test_reference_arm_xglobal():
     d = run_bench("--xglobal")
     check_common(d)
     assert "x-global" in d["metric"] and abs(d["vs_baseline"] - d["value"] / 197e3) < 1e-9
+
+
+def test_measured_traffic_rows_are_tied_to_the_cuda_sources(tmp_path, monkeypatch):
+    """profiles/dram_traffic.csv rows count only while their src_sha16 equals the hash of the CUDA sources being timed
+    ("stamp the CSV row with the hash it was captured at and refuse a mismatch")."""
+    sys.path.insert(0, ROOT)
+    import bench
+    sha = bench.source_sha16()
+    assert len(sha) == 16
+    prof = tmp_path / "profiles"
+    prof.mkdir()
+    (prof / "dram_traffic.csv").write_text(
+        "workload,kernel,dram_bytes_per_launch,planes_per_launch,src_sha16,source\n"
+        f"wl_a,k_plane_fused,1000,10,{sha},x\n"
+        "wl_b,k_plane_fused,2000,10,0123456789abcdef,x\n")
+    monkeypatch.setattr(bench, "ROOT", str(tmp_path))
+    monkeypatch.setattr(bench, "source_sha16", lambda: sha)
+    rows, why = bench.measured_traffic("wl_a")
+    assert why is None and rows == {"k_plane_fused": (1000.0, 10.0)}
+    rows, why = bench.measured_traffic("wl_b")
+    assert rows == {} and "predates" in why
+    rows, why = bench.measured_traffic("wl_c")
+    assert rows == {} and "no ncu capture" in why
