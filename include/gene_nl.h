@@ -167,6 +167,46 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind);
  */
 double gene_nl_query(const gene_nl_plan* h, int what);
 
+/*
+ * gene_nl_compute_static -- rhs += scale * N(chi, g) WITHOUT A PLAN AND WITHOUT ANY ALLOCATION (the same
+ * operation as gene_nl_compute with chi_has_v = 1: chi laid out like g, one chi plane per g plane).
+ *
+ * Why it exists.  gene_nl_create, gene_nl_set_* and the *_host entry points call cudaMalloc.  Some callers cannot:
+ * a code that gives all device memory to its own pool at start-up (a later cudaMalloc fails), a time-step loop running
+ * beside other streams (cudaMalloc / cudaFree synchronise the device and stall them), code inside a region where the
+ * runtime forbids allocation.  This call allocates no device memory and no pinned host memory: no cudaMalloc, cudaFree,
+ * cudaMallocHost, no stream or event creation.  The intermediate arrays of the planes in flight live in a
+ * `static __device__` array inside the library (33.75 MiB + 5 KiB), which every GPU that loads the library holds until
+ * the process exits, used or not.
+ *
+ * Limits (anything else returns GENE_NL_EUNSUPPORTED with a message that names the limit):
+ *   nx0 = GENE_NL_STATIC_NX0 (96) and nky0 = GENE_NL_STATIC_NKY0 (48) exactly, i.e. the 144 x 144 padded grid of
+ *   BASELINE.json configs[4]: the scratch is GENE_NL_STATIC_MAX_GROUPS (64) slots of 552 960 B, one per plane in flight,
+ *   and a larger plane does not fit a slot;  nz*nv*nw*nspec <= GENE_NL_STATIC_MAX_PLANES.
+ *   At most 64 SMs work (one plane each at a time): about 64/148 of the speed of gene_nl_compute on a B200.
+ * Arguments: extents, kxmin, kymin as gene_nl_create; chi, g, rhs: DEVICE pointers, caller-owned, 16-byte aligned,
+ * extents [nx0, nky0, nz, nv, nw, nspec], kx fastest (layout at the top of this file); rhs must not overlap chi or g.
+ * `stream`: cudaStream_t as void* (NULL = legacy default stream).  Asynchronous: a counter clear and one kernel are
+ * enqueued on `stream`; results equal gene_nl_compute's (same kernel code).  Errors as gene_nl_compute; on error before
+ * the launch rhs is untouched.
+ *
+ * First call on each device: it looks up the device addresses of the static arrays (cudaGetSymbolAddress), copies the
+ * root tables there with a synchronous cudaMemcpy and sets the kernel's shared-memory attribute, with that device
+ * current.  Make that first call outside any stream capture; later calls do none of this.
+ *
+ * Sharing: every call on a device uses the same static array and finds the previous call's contents in it.  Nothing a
+ * caller has to clear (the kernel overwrites each slot before reading it; the counters are cleared on `stream` by the
+ * call itself).  But two calls that OVERLAP on the GPU -- different streams, or host threads on the same device -- write
+ * the same slots and race: keep all calls on a device in one stream, or order them with events.  Plans
+ * (gene_nl_compute*) have their own scratch and may run concurrently with it.
+ */
+#define GENE_NL_STATIC_NX0 96
+#define GENE_NL_STATIC_NKY0 48
+#define GENE_NL_STATIC_MAX_GROUPS 64
+#define GENE_NL_STATIC_MAX_PLANES 2147483647LL
+int gene_nl_compute_static(int nx0, int nky0, int nz, int nv, int nw, int nspec, double kxmin, double kymin,
+                           const void* chi, const void* g, void* rhs, double scale, void* stream);
+
 /* =====================================================================================================
  * x-GLOBAL VARIANT -- the operator the paper itself ran and timed (PAPER.md:39,
  * sect. 2.1-2.3): spectral in y only, real space in x.  PAPER.md:61: the fields are transposed, extended

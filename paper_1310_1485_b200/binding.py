@@ -19,7 +19,7 @@ GENE_NL_OK, GENE_NL_EINVAL, GENE_NL_EUNSUPPORTED, GENE_NL_ECUDA, GENE_NL_ENOMEM 
 EXPORTED_SYMBOLS = (
     "gene_nl_create", "gene_nl_compute", "gene_nl_compute_em", "gene_nl_compute_host", "gene_nl_compute_em_host",
     "gene_nl_destroy", "gene_nl_last_error", "gene_nl_set_scratch_bytes", "gene_nl_set_plane_kernel",
-    "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query",
+    "gene_nl_workspace_bytes", "gene_nl_launches_per_compute", "gene_nl_query", "gene_nl_compute_static",
     "gene_nlx_create", "gene_nlx_compute", "gene_nlx_compute_host", "gene_nlx_destroy", "gene_nlx_query",
 )
 # ... and include/gene_nl_bench.h (benchmark-only helpers, not on the hot path)
@@ -74,6 +74,8 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_launches_per_compute.restype = i
         lib.gene_nl_query.argtypes = [vp, i]
         lib.gene_nl_query.restype = dbl
+        lib.gene_nl_compute_static.argtypes = [i, i, i, i, i, i, dbl, dbl, vp, vp, vp, dbl, vp]
+        lib.gene_nl_compute_static.restype = i
         lib.gene_nl_probe_peaks.argtypes = [ctypes.POINTER(dbl)]
         lib.gene_nl_probe_peaks.restype = i
         lib.gene_nl_probe_exchange.argtypes = [ctypes.POINTER(dbl)]
@@ -126,6 +128,28 @@ def gene_nl_compute(h, chi, g, rhs, scale, stream=None) -> None:
 
 
 GENE_NL_CHI_EM = 2
+GENE_NL_STATIC_NX0, GENE_NL_STATIC_NKY0, GENE_NL_STATIC_MAX_GROUPS = 96, 48, 64
+
+
+def gene_nl_compute_static(nx0, nky0, nz, nv, nw, nspec, kxmin, kymin, chi, g, rhs, scale, stream=None) -> None:
+    """rhs += scale*N(chi, g) with chi shaped like g, for callers that must not allocate device memory.
+
+    No plan: the library's other entry points cudaMalloc their tables and scratch, which a caller whose own pool
+    already owns the whole device, or whose other streams must not be stalled by cudaMalloc's device-wide
+    synchronisation, cannot afford.  This one keeps the planes in flight in a static device array inside the library
+    (33.75 MiB, held by every GPU that loads it) and supports planes of 96 x 48 modes only; anything else raises.
+    Calls on one device share that array: do not let two of them overlap on the GPU.  The first call per device
+    does a synchronous set-up (keep it outside stream capture).  See include/gene_nl.h."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    elif hasattr(stream, "cuda_stream"):
+        stream = stream.cuda_stream
+    rc = load_library().gene_nl_compute_static(int(nx0), int(nky0), int(nz), int(nv), int(nw), int(nspec), float(kxmin),
+                                               float(kymin), _ptr(chi), _ptr(g), _ptr(rhs), float(scale),
+                                               int(stream) or None)
+    if rc != GENE_NL_OK:
+        raise GeneNLError(f"gene_nl_compute_static failed ({rc}): {gene_nl_last_error()}")
 
 
 def gene_nl_compute_em(h, phi, apar, vpar, g, rhs, scale, stream=None) -> None:

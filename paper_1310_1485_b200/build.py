@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgene_nl.so")
-SOURCES = ["gene_nl.cu", "gene_nlx.cu", "probe.cu"]
+SOURCES = ["gene_nl.cu", "gene_nlx.cu", "gene_nl_static.cu", "probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--shared", "-cudart", "static"]
 
