@@ -261,7 +261,7 @@ def xglobal_main(args):
     traffic = cap["k_xglobal"][0] * wl.planes / cap["k_xglobal"][1] if "k_xglobal" in cap else None
     roofline = {"kernel": "k_xglobal", "bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s",
                 "frac": gbs / hbm_peak, "traffic": traffic,
-                "traffic_note": why or ("ncu dram__bytes capture of one whole step (profiles/r02_dram.md), stamped with src_sha16 %s" % source_sha16()),
+                "traffic_note": why or ("ncu dram__bytes capture of one whole step (profiles/r03_dram.md), stamped with src_sha16 %s" % source_sha16()),
                 "peak_source": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback 6650 GB/s",
                 "bytes_per_plane": B, "flops_per_plane": F, "achieved_tflops": F * wl.planes / (ms_per_step * 1e-3) / 1e12,
                 "share_of_step": 1.0}
@@ -431,6 +431,94 @@ def em_main(args):
         dist.destroy_process_group()
 
 
+def plane_kernel_name(wl, fused, kind, em=False):
+    """The instantiation gene_nl_create / gene_nl_set_plane_kernel selected for this plane shape (the tables find_fused2,
+    find_fused, find_group, find_wa, find_cluster of csrc/gene_nl.cu), from gene_nl_query(h, 7) and (h, 8): the roofline
+    line names the kernel that ran, not its class."""
+    nx, ny = wl.Nx, wl.Ny
+    chiv = bool(wl.chi_has_v) and not em
+    tail = ",EM" if em else (",CHIV" if chiv else "")
+    if not fused:
+        return None
+    if kind == 2.0:
+        return {(384, 192): "k_plane_group<24,16,24,G=4,NH=2%s>", (768, 384): "k_plane_group<48,16,24,G=8,NH=4,BY=16,X2=24x32%s>",
+                (144, 144): "k_plane_group<12,12,18,G=1%s>"}.get((nx, ny), "k_plane_group<?%s>") % tail
+    if kind == 4.0:
+        return {(384, 192): "k_plane_wa<24,16,24,8,G=4%s>", (768, 384): "k_plane_wa<24,32,24,16,G=8%s>",
+                (144, 144): "k_plane_wa<12,12,18,8,G=1%s>"}.get((nx, ny), "k_plane_wa<?%s>") % tail
+    if kind == 1.0:
+        return "k_plane_cluster<24,16,24,C=8>"
+    if ny == 96 and nx in (48, 96, 192):
+        return "k_plane_fused2<%d,12,8>" % (nx // 8)
+    return "k_plane_fused<%d,%d,8>" % (nx // 8, ny // 8)
+
+
+def side_xglobal(dev, peaks, planes=65536, steps=10):
+    """Device-resident x-global step on a slice of the paper's workload, for the compact summary of the
+    default run; `bench.py --xglobal` is the full measurement (589 824 planes, e2e, cpu_baseline)."""
+    import torch
+    from paper_1310_1485_b200 import gene_nlx_compute, gene_nlx_create, gene_nlx_destroy, gene_nlx_query
+    from paper_1310_1485_b200 import workloads as W
+    base = W.XGLOBAL_PAPER
+    wl = W.XGlobalWorkload(f"xglobal_64x16_{planes}", base.nx, base.nky0, planes, base.seed, base.scale)
+    arrs = W.make_xglobal_inputs(wl, dev)
+    h = gene_nlx_create(wl.nx, wl.nky0, wl.planes)
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        gene_nlx_compute(h, *arrs, wl.scale, stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        gene_nlx_compute(h, *arrs, wl.scale, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    gbs = gene_nlx_query(h, 5) * wl.planes / (ms * 1e-3) / 1e9
+    gene_nlx_destroy(h)
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    return {"kernel": "k_xglobal<48,6,8,64,16>", "bound": "hbm", "frac": gbs / hbm_peak, "achieved_gbs": gbs, "peak_gbs": hbm_peak,
+            "ms": ms, "planes": planes, "planes_per_s": planes / (ms * 1e-3), "gpu_launches": steps}
+
+
+def side_em(dev, idx=4, steps=5):
+    """Device-resident EM step (chi composed on the device) on configs[idx]'s grid, for the compact summary
+    of the default run; `bench.py --em` is the full measurement."""
+    import numpy as np
+    import torch
+    from paper_1310_1485_b200 import (GENE_NL_CHI_EM, gene_nl_compute_em, gene_nl_create, gene_nl_destroy,
+                                      gene_nl_launches_per_compute, gene_nl_query)
+    from paper_1310_1485_b200 import workloads as W
+    c = W.CONFIGS[idx]
+    wl = W.Workload(c.name + "_em_composed", c.nx0, c.nky0, c.nz, c.nv, c.nw, c.nspec, c.kxmin, c.kymin, False, c.seed,
+                    c.rhs_random, c.scale)
+    wl2 = W.Workload(wl.name + "_apar", c.nx0, c.nky0, c.nz, c.nv, c.nw, c.nspec, c.kxmin, c.kymin, False, c.seed + 77,
+                     c.rhs_random, c.scale)
+    vpar = np.concatenate([np.linspace(-3.0, 3.0, c.nv) * (1.0 + 0.5 * s) for s in range(c.nspec)])
+    phi, g, rhs = W.make_inputs(wl, dev)
+    apar = W.make_inputs(wl2, dev)[0]
+    h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        gene_nl_compute_em(h, phi, apar, vpar, g, rhs, wl.scale, stream)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        gene_nl_compute_em(h, phi, apar, vpar, g, rhs, wl.scale, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    fp64_model = 148 * FP64_LANES_PER_SM * 2 * 1.965e9 / 1e12
+    tf = gene_nl_query(h, 6) * wl.planes / (ms * 1e-3) / 1e12
+    name = plane_kernel_name(wl, gene_nl_query(h, 7) == 1.0, gene_nl_query(h, 8), em=True) or "k_xinv + k_ybracket<EM> + k_xfwd"
+    launches = gene_nl_launches_per_compute(h) * steps
+    gene_nl_destroy(h)
+    return {"kernel": name, "bound": "alu", "step_frac": tf / fp64_model, "achieved_tflops": tf, "ms": ms, "planes": wl.planes,
+            "planes_per_s": wl.planes / (ms * 1e-3), "gpu_launches": launches,
+            "note": "whole step incl. the chi-side launches on phi_bar and A_par_bar"}
+
+
 def source_sha16():
     """sha256 over the CUDA sources: rows of profiles/dram_traffic.csv are stamped with it at capture time."""
     import hashlib
@@ -558,16 +646,17 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
                           "tflops": flops[k] * nprof / (prof_ms[k] * 1e-3) / 1e12}
     dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
     # measured DRAM bytes (ncu capture of these very sources; null when the capture is older than the code)
-    cap, why = measured_traffic(wl.name + ({1: "+cluster", 3: "+batched"}.get(plane_kernel, "")))
+    cap, why = measured_traffic(wl.name + ({1: "+cluster", 3: "+batched", 4: "+warp"}.get(plane_kernel, "")))
     traffic = cap[dom][0] if dom in cap else None
     traffic_step = None
     if cap and all(k in cap for k in kernels):
         # whole step: every kernel class's captured bytes per launch (average over the launches of one step of the full
         # workload) x the launches this run made per step
         traffic_step = sum(cap[k][0] * kernels[k]["launches_per_step"] for k in kernels)
-    roofline = {"kernel": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
+    kname = plane_kernel_name(my, nl.query(7) == 1.0, nl.query(8)) if dom == "k_plane_fused" else None
+    roofline = {"kernel": kname or dom, "kernel_class": dom, "bound": "alu", "achieved": kernels[dom]["tflops"], "peak": fp64_model,
                 "unit": "TFLOP/s", "frac": kernels[dom]["tflops"] / fp64_model, "traffic": traffic,
-                "traffic_note": why or ("ncu dram__bytes capture of one whole step (profiles/r02_dram.md), stamped with src_sha16 %s" % source_sha16()),
+                "traffic_note": why or ("ncu dram__bytes capture of one whole step (profiles/r03_dram.md), stamped with src_sha16 %s" % source_sha16()),
                 "peak_source": "model 148 SM x 64 FP64 lanes x 2 x 1.965 GHz (DESIGN.md sect. 7)",
                 "peak_measured_dfma": probe_tf, "smem_gbs_measured": probe_smem_gbs,
                 "share_of_step": kernels[dom]["ms_per_step"] / sum(v["ms_per_step"] for v in kernels.values())}
@@ -633,7 +722,8 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
                         "sample": f"{n} planes of {wl.name} (first planes, up to four (w,s) slabs), {dt:.1f} s wall"}
     return {
         "value": value, "steps": steps, "warmup": warm, "ms_per_step": ms_per_step, "scaling": "strong" if strong else "weak",
-        "config": {"workload": wl.name, "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": my.planes,
+        "config": {"workload": wl.name, "configs_index": [c.name for c in W.CONFIGS].index(wl.name) if wl in W.CONFIGS else None,
+                   "nx0": wl.nx0, "nky0": wl.nky0, "planes_per_gpu": my.planes,
                    "padded_grid": [wl.Nx, wl.Ny], "chi_has_v": wl.chi_has_v,
                    "cache": "inputs larger than L2 (g+rhs+chi = %.0f MiB per GPU)" %
                             ((2 * my.planes + my.chi_planes) * my.plane_bytes / 2 ** 20),
@@ -726,6 +816,24 @@ def main():
             r = run_config(W.CONFIGS[2], args, env, do_e2e=False, do_cpu=False, headline=False, plane_kernel=kind)
             per_config[W.CONFIGS[2].name + f" (gene_nl_set_plane_kernel: {label})"] = {
                 k: r[k] for k in ("value", "ms_per_step", "steps", "roofline", "roofline_step", "kernels", "clocks", "gpu_launches")}
+    if per_config is not None:
+        # compact summary where the driver's parsed record keeps it (inside `roofline`): every target configuration with the
+        # kernel that ran, plus one device-resident line each for the x-global operator (f2) and the composed-chi operator (f1)
+        def brief(r):
+            return {"kernel": r["roofline"]["kernel"], "frac": r["roofline"]["frac"], "step_frac": r["roofline_step"]["frac"],
+                    "ms": r["ms_per_step"], "planes_per_s": r["value"]}
+        summary = {wl.name: brief(res)}
+        for name, r in per_config.items():
+            summary[name] = brief(r)
+        extra_launches = 0
+        for key, fn in (("xglobal_64x16_65536", lambda: side_xglobal(dev, peaks)), ("cfg4_em_96x48_em_composed", lambda: side_em(dev))):
+            try:
+                summary[key] = fn()
+                extra_launches += summary[key].pop("gpu_launches", 0)
+            except Exception as e:  # noqa: BLE001  (a side line must not cost the headline)
+                summary[key] = {"error": str(e)[:200]}
+            torch.cuda.empty_cache()
+        res["roofline"]["per_config"] = summary
     if rank == 0:
         line = {
             "metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": res["steps"],

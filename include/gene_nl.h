@@ -81,8 +81,9 @@ int gene_nl_compute(gene_nl_plan* h, const void* chi, const void* g, void* rhs, 
  * a call first waits on the host for the previous call's copy, and the call is NOT capturable in a CUDA graph
  * (gene_nl_compute is).  By linearity the two fields are transformed to real space once per (z,w,s) and combined
  * inside the bracket kernel, so the per-plane chi array (as large as g) is never formed, read or transformed.  Other
- * arguments, errors and asynchrony as gene_nl_compute.  Always the batched kernels.  gene_nl_compute /
- * gene_nl_compute_host reject such a plan.
+ * arguments, errors and asynchrony as gene_nl_compute.  The group kernel composes chi where it exists (384 x 192 and
+ * 144 x 144 padded grids), else the batched bracket kernel does.  Called while `stream` is being captured it returns
+ * GENE_NL_EUNSUPPORTED and leaves the capture intact.  gene_nl_compute / gene_nl_compute_host reject such a plan.
  */
 #define GENE_NL_CHI_EM 2
 int gene_nl_compute_em(gene_nl_plan* h, const void* phi, const void* apar, const double* vpar_host, const void* g,
@@ -110,7 +111,9 @@ void gene_nl_destroy(gene_nl_plan* h);
 /* Thread-local description of the last failure in this library ("" if none). */
 const char* gene_nl_last_error(void);
 
-/* Bytes of device scratch + tables owned by the plan. */
+/* Bytes of device memory owned by the plan: root tables, the Z / P / R scratch set, the group kernel's per-group
+ * scratch and hand-over counters, the v_par coefficients of an EM plan.  (The staging buffers the *_host entry points
+ * create on first use are not counted.) */
 size_t gene_nl_workspace_bytes(const gene_nl_plan* h);
 
 /*
@@ -131,21 +134,26 @@ int gene_nl_launches_per_compute(const gene_nl_plan* h);
  *   GENE_NL_KERNEL_AUTO     what gene_nl_create selected (the fastest measured on B200): the fused shared-memory kernel
  *                           for planes that fit one SM; beyond that the group kernel where it exists, else the batched
  *                           kernels.
- *   GENE_NL_KERNEL_GROUP    the fused kernel spread over groups of 4 co-resident CTAs (one cooperative launch, every SM
+ *   GENE_NL_KERNEL_GROUP    the fused kernel spread over groups of G co-resident CTAs (one cooperative launch, every SM
  *                           used): the two x<->y hand-overs of a plane (the "transpositions" of PAPER.md:61) go through
- *                           a per-group scratch of 1.1 MB that is rewritten every plane and therefore stays in L2; rows
- *                           come back by 1-D bulk copies (TMA).  HBM sees g, rhs and the chi rows only (1.07 x the
- *                           algorithmic bytes).  Exists for the 384 x 192 padded grid (nx0 = 256, nky0 = 64:
- *                           configs[2]) with chi_has_v = 0 on a device with cooperative launch.
+ *                           a per-group scratch that is rewritten every plane and therefore stays in L2; rows come
+ *                           back by 1-D bulk copies (TMA).  HBM sees g, rhs and the chi rows only (1.02 - 1.46 x the
+ *                           algorithmic bytes).  Exists, on a device with cooperative launch, for the padded grids
+ *                             384 x 192 (nx0 = 256, nky0 = 64: configs[2])  G = 4, chi_has_v = 0 or GENE_NL_CHI_EM,
+ *                             768 x 384 (nx0 = 512, nky0 = 128: configs[3]) G = 8, chi_has_v = 0,
+ *                             144 x 144 (nx0 = 96, nky0 = 48: configs[4])   G = 1, chi_has_v = 0, 1 or GENE_NL_CHI_EM
+ *                           (with chi_has_v = 1 chi goes through the same kernel: one launch per compute).
  *   GENE_NL_KERNEL_CLUSTER  the same phases over a thread-block cluster of 8 CTAs with the half-transformed plane in the
  *                           cluster's shared memory and distributed-shared-memory hand-overs (1.03 x the algorithmic
- *                           bytes; slower: DSMEM stores run at 18 B/clk/SM and 15 clusters fit the 148 SMs).  Same sizes.
+ *                           bytes; slower: DSMEM stores run at 18 B/clk/SM and 15 clusters fit the 148 SMs).  384 x 192
+ *                           with chi_has_v = 0 only.
  *   GENE_NL_KERNEL_BATCHED  the batched kernels (scratch through HBM/L2 in large batches) whatever the size.
  *   GENE_NL_KERNEL_WARP     the group kernel with warp-autonomous x phases as well (a warp takes two adjacent columns
  *                           through both x stages in its own shared-memory tile; every warp arrives on the hand-over
  *                           counters; no CTA-wide barrier in the plane loop).  Measured on B200: 3 % faster than the
  *                           group kernel at 384 x 192, 10 % slower at 768 x 384 and 144 x 144 (DESIGN.md sect. 6g), so
- *                           it is an option, not the default.  Same sizes as the group kernel, not with GENE_NL_CHI_EM.
+ *                           it is an option, not the default.  384 x 192 and 768 x 384 with chi_has_v = 0, 144 x 144
+ *                           with chi_has_v = 0 or 1; not with GENE_NL_CHI_EM.
  * GENE_NL_EUNSUPPORTED when the plan has no such kernel.  Same results to rounding (all are checked against the
  * oracle).  Synchronises the device and re-allocates the scratch, like gene_nl_set_scratch_bytes.
  */

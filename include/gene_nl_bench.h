@@ -35,17 +35,6 @@ int gene_nl_compute_profiled(gene_nl_plan* h, const void* chi, const void* g, vo
  */
 int gene_nl_probe_peaks(double* out3);
 
-/*
- * gene_nl_probe_exchange -- the exchange of complex128 values between the lanes of a warp (the step between two
- * register-resident FFT stages) next to the FP64 work of one radix-8 butterfly per 8 values.  With 8 warps per SM:
- * out[0] = ns per iteration for the FMAs alone, out[1] = with the exchange through a per-warp shared-memory tile
- * (8 STS.128 + 8 LDS.128 per lane), out[2] = with the exchange by warp shuffles (32 SHFL per lane); out[3..5] = the same
- * with 16 warps per SM, per 8 warps; out[6..8] = the same with 8 warps per SM and twice the FP64 work per exchange (tells
- * a shared-memory bandwidth bound from a serialisation of the two pipes).  SURVEY.md sect. 7 asked for this measurement before relying on "warp-shuffle
- * butterflies" (north_star); DESIGN.md sect. 6h has the result.
- */
-int gene_nl_probe_exchange(double* out9);
-
 #ifdef __cplusplus
 }
 #endif

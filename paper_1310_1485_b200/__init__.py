@@ -9,7 +9,7 @@ from . import workloads  # noqa: F401
 _BINDING_NAMES = (
     "gene_nl_create", "gene_nl_compute", "gene_nl_compute_em", "gene_nl_destroy", "gene_nl_last_error", "GENE_NL_CHI_EM",
     "gene_nl_compute_host", "gene_nl_compute_em_host", "gene_nl_set_scratch_bytes", "gene_nl_set_plane_kernel", "GENE_NL_KERNEL_AUTO", "GENE_NL_KERNEL_CLUSTER", "GENE_NL_KERNEL_GROUP", "GENE_NL_KERNEL_BATCHED", "GENE_NL_KERNEL_WARP", "gene_nl_compute_profiled", "gene_nl_workspace_bytes", "gene_nl_launches_per_compute",
-    "gene_nl_query", "gene_nl_compute_static", "gene_nl_probe_peaks", "gene_nl_probe_exchange", "GeneNL", "GeneNLError", "library_path", "load_library",
+    "gene_nl_query", "gene_nl_compute_static", "gene_nl_probe_peaks", "GeneNL", "GeneNLError", "library_path", "load_library",
     "gene_nlx_create", "gene_nlx_compute", "gene_nlx_compute_host", "gene_nlx_destroy", "gene_nlx_query",
 )
 

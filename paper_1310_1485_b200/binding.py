@@ -23,7 +23,7 @@ EXPORTED_SYMBOLS = (
     "gene_nlx_create", "gene_nlx_compute", "gene_nlx_compute_host", "gene_nlx_destroy", "gene_nlx_query",
 )
 # ... and include/gene_nl_bench.h (benchmark-only helpers, not on the hot path)
-BENCH_SYMBOLS = ("gene_nl_compute_profiled", "gene_nl_probe_peaks", "gene_nl_probe_exchange")
+BENCH_SYMBOLS = ("gene_nl_compute_profiled", "gene_nl_probe_peaks")
 
 _lock = threading.Lock()
 _lib = None
@@ -78,8 +78,6 @@ def load_library() -> ctypes.CDLL:
         lib.gene_nl_compute_static.restype = i
         lib.gene_nl_probe_peaks.argtypes = [ctypes.POINTER(dbl)]
         lib.gene_nl_probe_peaks.restype = i
-        lib.gene_nl_probe_exchange.argtypes = [ctypes.POINTER(dbl)]
-        lib.gene_nl_probe_exchange.restype = i
         ll = ctypes.c_longlong
         lib.gene_nlx_create.argtypes = [i, i, ll]
         lib.gene_nlx_create.restype = vp
@@ -187,7 +185,8 @@ GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_CLUSTER, GENE_NL_KERNEL_GROUP, GENE_NL_KERNE
 
 
 def gene_nl_set_plane_kernel(h, kind: int) -> None:
-    """Kernel family for the g side of a plane: GENE_NL_KERNEL_AUTO or GENE_NL_KERNEL_CLUSTER (see include/gene_nl.h)."""
+    """Kernel family for the g side of a plane: GENE_NL_KERNEL_AUTO, _GROUP (384 x 192, 768 x 384, 144 x 144 padded
+    grids), _WARP (the same grids, not EM), _CLUSTER (384 x 192) or _BATCHED (any size); see include/gene_nl.h."""
     rc = load_library().gene_nl_set_plane_kernel(h, int(kind))
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_set_plane_kernel failed ({rc}): {gene_nl_last_error()}")
@@ -243,16 +242,6 @@ def gene_nl_probe_peaks():
     if rc != GENE_NL_OK:
         raise GeneNLError(f"gene_nl_probe_peaks failed ({rc})")
     return float(out[0]), float(out[1]), float(out[2])
-
-
-def gene_nl_probe_exchange():
-    """ns per iteration and 8 warps of (FP64 butterflies alone, + exchange through shared memory, + exchange by warp
-    shuffles) with 8 warps per SM, the same three with 16 warps per SM, and with 8 warps and twice the FP64 work."""
-    out = (ctypes.c_double * 9)()
-    rc = load_library().gene_nl_probe_exchange(out)
-    if rc != GENE_NL_OK:
-        raise GeneNLError(f"gene_nl_probe_exchange failed ({rc})")
-    return tuple(float(v) for v in out)
 
 
 # ---- x-global variant (include/gene_nl.h, gene_nlx_*) ----

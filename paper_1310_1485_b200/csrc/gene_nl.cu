@@ -305,6 +305,7 @@ struct Scratch {
     cplx *Z = nullptr, *P = nullptr, *R = nullptr;
     cplx* GS = nullptr;       // group kernel: Z + P of every group's current plane (L2 resident)
     unsigned* cnt = nullptr;  // group kernel: two hand-over counters per group
+    size_t r2off = 0;         // em on a plane kernel: where A_par_bar's real-space fields start in R (in values)
 };
 
 // Optional per-launch CUDA-event timing (gene_nl_compute_profiled): kernel classes
@@ -387,6 +388,7 @@ bool alloc_scratch(size_t zbytes, size_t pbytes, size_t rbytes, Scratch* s)
     if (!cuda_ok(cudaMalloc(&s->Z, zbytes), "cudaMalloc(Z)")) return false;
     if (!cuda_ok(cudaMalloc(&s->P, pbytes), "cudaMalloc(P)")) return false;
     if (!cuda_ok(cudaMalloc(&s->R, rbytes), "cudaMalloc(Rchi)")) return false;
+    s->r2off = rbytes / (2 * sizeof(cplx));   // em: phi_bar's fields fill the first half, A_par_bar's the second
     return true;
 }
 bool alloc_scratch(gene_nl_plan* h, Scratch* s);
@@ -608,7 +610,7 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
                 GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, s.R + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
                 launches += 2;
                 if (apar) {  // em: the same two kernels on A_par_bar; its real-space fields fill the second half of R
-                    cplx* R2 = s.R + h->rbytes / (2 * sizeof(cplx));
+                    cplx* R2 = s.R + s.r2off;
                     GNL_XINV(prof, st, nb * xt, apar + (size_t)s0 * cps * h->M + q0 * h->M, s.Z, nb, 0);
                     GNL_LAUNCH(prof, K_YREAL, (yk.real<<<nb * yt_rows, yk.nt, yk.smem_real, st>>>(s.Z, R2 + q0 * (size_t)h->Nx * h->Ny, h->twy, h->Nx)));
                     launches += 2;
@@ -634,7 +636,7 @@ int enqueue_slabs(gene_nl_plan* h, const Scratch& s, const cplx* chi, const cplx
                 // (a persisting-L2 access window over the scratch was measured on B200: the kernel gains 1.5 %, the
                 // chi-side kernels lose more to the carve-out: not used)
                 GNL_LAUNCH(prof, K_FUSED, (cudaLaunchKernelEx(&cfg, h->fk.fng, g + goff, (cplx*)(rhs + goff), (const cplx*)s.R, (const cplx*)(h->fk.chiv ? chi + goff : nullptr), (const cplx*)h->twx, (const cplx*)h->twy, s.GS, s.cnt, h->nz, h->nv, ns, h->kxmin, h->kymin, coef,
-                                                              (const cplx*)(apar ? s.R + h->rbytes / (2 * sizeof(cplx)) : nullptr), (const double*)(apar ? h->vp_dev : nullptr), h->nw, slab0 + s0)));
+                                                              (const cplx*)(apar ? s.R + s.r2off : nullptr), (const double*)(apar ? h->vp_dev : nullptr), h->nw, slab0 + s0)));
             } else if (h->fk.fnc) {
                 // whole clusters only; a cluster walks planes with the stride of the cluster count
                 const int C = h->fk.cluster;
@@ -797,6 +799,10 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             h->wk_grid = (sms / h->wk.group) * h->wk.group;
         }
     }
+    // The two optimisations of the batched path further down are decided for the batched path itself, i.e. for every
+    // plane that does not fit one SM, whether or not a group kernel becomes the default next: enqueue_chunk consults them
+    // only when the batched kernels run (gene_nl_set_plane_kernel(GENE_NL_KERNEL_BATCHED) on such a plan included).
+    const bool one_sm = h->fused;
     if (ok && h->gk.fng && !h->fused) {
         // Planes beyond one SM with chi shared over v: the group kernel (Z and P through L2) is the default where it
         // exists.  Measured on B200 at configs[2]: 6.24 ms per step against 7.24 ms for the batched kernels and 8.18 ms
@@ -816,7 +822,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, h->xk.invp, h->xk.nt, h->xk.smem_invp) == cudaSuccess && occ > 0)
             h->xk.cap_invp = occ * sms;
     }
-    if (ok && !h->chi_has_v && !h->em && !h->fused && (h->Nx / 2) % h->yk.rp_t == 0 && h->nky0 % h->xk.ck_zt == 0 &&
+    if (ok && !h->chi_has_v && !h->em && !one_sm && (h->Nx / 2) % h->yk.rp_t == 0 && h->nky0 % h->xk.ck_zt == 0 &&
         h->Ny <= 192 && h->yk.smem_t <= 227 * 1024 && h->xk.smem_invp_zt <= 227 * 1024) {
         // measured on B200: 384 x 192 (configs[2]) 7.79 -> 7.19 ms; at Ny = 384 the 105 KB of exchange tiles of
         // k_ybracket_t cost more than the stores save (configs[3]: 101 -> 119 ms), so that size keeps the row-major Z
@@ -829,7 +835,7 @@ gene_nl_plan* gene_nl_create(int nx0, int nky0, int nz, int nv, int nw, int nspe
             h->cap_invp_zt = occ * sms;
         }
     }
-    if (ok && h->chi_has_v && !h->fused && (h->Nx / 2) % h->yk.rp_cv == 0 && h->yk.smem_cv <= 227 * 1024)
+    if (ok && h->chi_has_v && !one_sm && (h->Nx / 2) % h->yk.rp_cv == 0 && h->yk.smem_cv <= 227 * 1024)
         h->fuse_chi_y = set_smem(h->yk.br_cv, h->yk.smem_cv, "k_ybracket_cv smem");
     if (!ok) {
         std::string keep = g_err;
@@ -916,7 +922,7 @@ int gene_nl_set_plane_kernel(gene_nl_plan* h, int kind)
         return GENE_NL_EINVAL;
     }
     if (kind == GENE_NL_KERNEL_GROUP && !h->gk.fng) {
-        set_err("gene_nl_set_plane_kernel: no group kernel for this plan (384 x 192 padded grid, chi shared over v, cooperative launch)");
+        set_err("gene_nl_set_plane_kernel: no group kernel for this plan (padded grids 384 x 192 [chi_has_v = 0 or EM], 768 x 384 [chi_has_v = 0], 144 x 144 [any chi]; a device with cooperative launch)");
         return GENE_NL_EUNSUPPORTED;
     }
     if (kind == GENE_NL_KERNEL_WARP && !h->wk.fng) {
@@ -1005,6 +1011,13 @@ int gene_nl_compute_em(gene_nl_plan* h, const void* phi_, const void* apar_, con
     if (!rc) rc = check_ptrs(apar_, g_, rhs_, gbytes, cbytes);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone) {
+        // (the host wait on the pinned v_par staging buffer would invalidate the capture)
+        set_err("gene_nl_compute_em cannot be captured in a CUDA graph (host-side staging of v_par); gene_nl_compute can");
+        return GENE_NL_EUNSUPPORTED;
+    }
+    cudaGetLastError();
     rc = stage_vpar(h, vpar_host, st);
     if (rc) return rc;
     if (enqueue_slabs(h, h->scr, (const cplx*)phi_, (const cplx*)g_, (cplx*)rhs_, h->nw * h->nspec, scale, st, nullptr,
@@ -1055,8 +1068,9 @@ static int host_impl(gene_nl_plan* h, const void* chi_, const void* apar_, const
         // built locally and moved into the plan only when every allocation succeeded
         const int nstage = 3;
         std::vector<HostStage> st(nstage);
-        size_t rbytes1 = h->rbytes;  // a stage's scratch set serves one slab
-        if (h->fused && !h->em) rbytes1 = sizeof(cplx) * (size_t)h->Nx * h->Ny * (size_t)h->nz * (h->chi_has_v ? h->nv : 1);
+        size_t rbytes1 = h->rbytes;  // a stage's scratch set serves ONE slab: its real-space chi fields (em: of both
+        if (h->fused)                // potentials; chi through the plane kernel: none), not those of a launch of nss slabs
+            rbytes1 = h->fk.chiv ? 256 : sizeof(cplx) * (size_t)h->Nx * h->Ny * (size_t)h->nz * (h->chi_has_v ? h->nv : 1) * (h->em ? 2 : 1);
         bool ok = true;
         for (auto& s : st) {
             ok = ok && cuda_ok(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking), "cudaStreamCreate") &&
@@ -1127,7 +1141,13 @@ int gene_nl_compute_em_host(gene_nl_plan* h, const void* phi_, const void* apar_
 size_t gene_nl_workspace_bytes(const gene_nl_plan* h)
 {
     if (!h) return 0;
-    return h->zbytes + h->pbytes + h->rbytes + h->table_bytes;
+    size_t n = h->zbytes + h->pbytes + h->rbytes + h->table_bytes;
+    if (h->fused && h->fk.fng) {   // the group kernel's L2-resident scratch and its hand-over counters
+        const size_t ngroup = (size_t)(h->fused_grid / h->fk.group);
+        n += h->fk.group_scratch * ngroup + sizeof(unsigned) * 2 * ngroup;
+    }
+    if (h->em) n += sizeof(double) * (size_t)h->nv * h->nspec;
+    return n;
 }
 
 int gene_nl_launches_per_compute(const gene_nl_plan* h)

@@ -549,9 +549,15 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     }
                     // the +ky halves of these P rows (one 128-byte line per row and unit, read by this warp instruction only)
                     // are dead: drop them from L2 where the groups' scratch exceeds what L2 keeps
-                    if (K::DISCARD && CK == 8 && col == 0) {
+                    if constexpr (K::DISCARD && CK == 8) {
+                        // the other seven lanes of the line have their values too before it is dropped (whole warps run
+                        // this loop, so the warp barrier is met by all 32 lanes)
+                        static_assert((UPP * CK * AX2) % 32 == 0, "whole warps in the stage-1 loop of X2");
+                        __syncwarp(FULL);
+                        if (col == 0) {
 #pragma unroll
-                        for (int i = 0; i < C22; ++i) l2_discard_line(Ps + (size_t)(n1 + AX2 * i) * W2 + kyi);
+                            for (int i = 0; i < C22; ++i) l2_discard_line(Ps + (size_t)(n1 + AX2 * i) * W2 + kyi);
+                        }
                     }
                 }
                 cplx* Rcol = Rb + (size_t)((rank + G * (ub + us)) * CK + cols) * NX0 + k2s;

@@ -48,93 +48,7 @@ __global__ void __launch_bounds__(256) k_probe_smem(double* out, int iters)
     out[blockIdx.x * blockDim.x + t] = x + y;
 }
 
-// Exchange of complex128 values between the lanes of a warp, the step between two register-resident FFT stages, next to
-// FP64 work of about one radix-8 butterfly per 8 values ("Warp shuffles of FP64 data are 2x32-bit shuffles
-// per double ... measure before relying on warp-shuffle butterflies").  MODE 0: the FMAs alone; 1: + exchange through a
-// per-warp shared-memory tile (8 x STS.128, 8 x LDS.128, conflict free); 2: + exchange by shuffles (8 x 4 SHFL.BFLY).
-template <int MODE, int U>
-__global__ void __launch_bounds__(256) k_probe_xchg(double* out, int iters, double b, double c)
-{
-    extern __shared__ double2 buf[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double2* tile = buf + warp * (8 * 33);
-    double2 v[8];
-#pragma unroll
-    for (int j = 0; j < 8; ++j) v[j] = make_double2(1.0 + 1e-3 * (lane + 32 * j), 0.5 - 1e-3 * j);
-    for (int it = 0; it < iters; ++it) {
-#pragma unroll
-        for (int u = 0; u < U; ++u) {   // U = 5: 80 FP64 instructions per 8 values (a twiddled radix 8 has 76)
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                v[j].x = fma(v[j].x, b, c);
-                v[j].y = fma(v[j].y, b, -c);
-            }
-        }
-        if (MODE == 1) {
-#pragma unroll
-            for (int j = 0; j < 8; ++j) tile[j * 33 + lane] = v[j];
-            __syncwarp();
-#pragma unroll
-            for (int j = 0; j < 8; ++j) v[j] = tile[j * 33 + ((lane + 1 + j) & 31)];
-            __syncwarp();
-        } else if (MODE == 2) {
-#pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                v[j].x = __shfl_xor_sync(0xffffffffu, v[j].x, j + 1);
-                v[j].y = __shfl_xor_sync(0xffffffffu, v[j].y, j + 1);
-            }
-        }
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int j = 0; j < 8; ++j) s += v[j].x + v[j].y;
-    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
-}
-
 }  // namespace
-
-extern "C" int gene_nl_probe_exchange(double* out9)
-{
-    if (!out9) return GENE_NL_EINVAL;
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return GENE_NL_ECUDA;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const int threads = 256, iters = 4096;   // 8 warps per SM, as the plane kernels; then 16 (two CTAs per SM)
-    const size_t smem = sizeof(double2) * 8 * (8 * 33);
-    double* buf = nullptr;
-    if (cudaMalloc(&buf, sizeof(double) * 2 * sms * threads) != cudaSuccess) return GENE_NL_ENOMEM;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0);
-    cudaEventCreate(&e1);
-    for (int cfg = 0; cfg < 3; ++cfg)   // 8 warps per SM; 16 warps per SM; 8 warps per SM with twice the FP64 work
-    for (int mode = 0; mode < 3; ++mode) {
-        const int occ = cfg == 1 ? 2 : 1;
-        const int blocks = occ * sms;
-        float best = 1e30f, ms = 0.f;
-        for (int rep = 0; rep < 4; ++rep) {
-            cudaEventRecord(e0);
-            if (cfg < 2) {
-                if (mode == 0) k_probe_xchg<0, 5><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-                else if (mode == 1) k_probe_xchg<1, 5><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-                else k_probe_xchg<2, 5><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-            } else {
-                if (mode == 0) k_probe_xchg<0, 10><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-                else if (mode == 1) k_probe_xchg<1, 10><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-                else k_probe_xchg<2, 10><<<blocks, threads, smem>>>(buf, iters, 1.0000001, 1e-9);
-            }
-            cudaEventRecord(e1);
-            cudaEventSynchronize(e1);
-            cudaEventElapsedTime(&ms, e0, e1);
-            if (rep > 0 && ms < best) best = ms;
-        }
-        out9[3 * cfg + mode] = (double)best * 1e6 / iters / occ;   // ns per iteration (8 values per lane) and 8 warps of an SM
-    }
-    cudaError_t err = cudaDeviceSynchronize();
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(buf);
-    return err == cudaSuccess ? GENE_NL_OK : GENE_NL_ECUDA;
-}
 
 extern "C" int gene_nl_probe_peaks(double* out3)
 {

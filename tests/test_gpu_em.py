@@ -61,6 +61,9 @@ def run_em(wl, phi, apar, vpar, g, rhs, scratch_bytes=None, host=False, plane_ke
 
 
 SHAPES = [(16, 8, 3, 5, 2, 2), (64, 32, 2, 3, 2, 1), (96, 48, 2, 4, 1, 2), (96, 48, 3, 5, 3, 2), (128, 32, 3, 3, 1, 1),
+          (96, 48, 8, 10, 2, 2),    # 320 planes > 2 x 148 groups of one CTA: every group walks on to a second and third
+                                    # plane, and v_par's species index changes inside a group's walk
+          (256, 64, 4, 5, 3, 2),    # 120 planes > 3 x 37 groups of four CTAs
           (256, 64, 2, 2, 1, 2), (256, 64, 2, 3, 3, 2),
           (32, 128, 1, 3, 1, 1),
           (256, 64, 36, 2, 1, 1)]   # chi rows of a chunk beyond 40 MB: k_ybracket<EM> walks its tiles v-fastest
@@ -110,6 +113,62 @@ def test_em_host_entry_point_matches_the_device_entry_point(cuda_device):
         G, R = (W.as_planes(t, wl).cpu().numpy() for t in (g, rhs))
         ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
         assert plane_errors(wl, W.as_planes(hst, wl).cpu().numpy(), ref, R).max() <= TOL
+
+
+def test_em_full_size_config4_grid_sampled_planes(cuda_device):
+    """The run BASELINE.md quotes (bench.py --em): configs[4]'s grid, 73 728 planes, phi_bar and A_par_bar supplied and chi
+    composed in the group kernel; >= 160 sampled planes (both ends, every (w,s) slab) against the oracle on chi composed
+    in numpy for those planes."""
+    from helpers import plane_max_errors, sample_planes
+    c4 = W.CONFIGS[4]
+    wl = W.Workload("cfg4_em_composed", c4.nx0, c4.nky0, c4.nz, c4.nv, c4.nw, c4.nspec, c4.kxmin, c4.kymin, False,
+                    c4.seed, c4.rhs_random, c4.scale)
+    need = 16 * wl.nx0 * wl.nky0 * 3.3 * wl.planes
+    torch.cuda.empty_cache()
+    if torch.cuda.mem_get_info()[0] < need:
+        pytest.skip(f"{wl.name} needs {need / 2**30:.0f} GiB of device memory")
+    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+    out = run_em(wl, phi, apar, vpar, g, rhs)
+    planes = sample_planes(wl, 160, wl.seed)
+    X, A = (W.as_planes(t, wl) for t in (phi, apar))
+    chi = np.empty((len(planes), wl.nky0, wl.nx0), complex)
+    for i, p in enumerate(planes):
+        p = int(p)
+        z, v, ws = p % wl.nz, (p // wl.nz) % wl.nv, p // (wl.nz * wl.nv)
+        q = z + wl.nz * ws
+        chi[i] = X[q].cpu().numpy() - vpar[v + wl.nv * (ws // wl.nw)] * A[q].cpu().numpy()
+    idx = torch.as_tensor(planes, dtype=torch.long, device=g.device)
+    G, R, got = (W.as_planes(t, wl)[idx].cpu().numpy() for t in (g, rhs, out))
+    ref = oracle.nl_pseudospectral(chi, G, R, wl.scale, wl.kxmin, wl.kymin)
+    assert plane_errors(wl, got, ref, R).max() <= TOL
+    assert plane_max_errors(wl, got, ref, R).max() <= TOL
+    h = wl.nx0 // 2
+    assert torch.equal(W.as_planes(out, wl)[:, :, h], W.as_planes(rhs, wl)[:, :, h])
+
+
+def test_em_refuses_stream_capture_and_leaves_the_capture_intact(cuda_device):
+    """gene_nl_compute_em stages v_par through a pinned host buffer and waits on the host for the previous copy, which a
+    capturing stream does not allow: the call says so (GENE_NL_EUNSUPPORTED) instead of breaking the caller's capture."""
+    from paper_1310_1485_b200 import GENE_NL_CHI_EM, GeneNLError, gene_nl_compute_em, gene_nl_create, gene_nl_destroy
+    wl = W.small_workload(96, 48, 2, 2, 1, 1, 0.1, 0.1, False, seed=9)
+    phi, apar, vpar, g, rhs = em_inputs(wl, cuda_device)
+    out = rhs.clone()
+    h = gene_nl_create(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, GENE_NL_CHI_EM)
+    try:
+        gene_nl_compute_em(h, phi, apar, vpar, g, out, wl.scale)
+        torch.cuda.synchronize()
+        expect = out.clone()
+        x = torch.zeros(8, device=cuda_device)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            with pytest.raises(GeneNLError, match="captured"):
+                gene_nl_compute_em(h, phi, apar, vpar, g, out, wl.scale)
+            x.add_(1.0)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert x.eq(1.0).all() and torch.equal(out, expect)
+    finally:
+        gene_nl_destroy(h)
 
 
 def test_em_errors(cuda_device):

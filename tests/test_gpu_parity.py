@@ -35,11 +35,14 @@ SHAPES = [
     (128, 32, 3, 3, 1, 1, False), (128, 64, 1, 2, 1, 1, True),
     (256, 64, 2, 2, 1, 1, False), (32, 128, 1, 3, 1, 1, False),
     (512, 16, 1, 2, 1, 1, True), (16, 8, 1, 1, 1, 1, False),
-    (256, 64, 36, 2, 1, 1, False),   # chi rows of a chunk beyond 40 MB: the v-fastest tile walk of k_ybracket_t
+    (256, 64, 36, 2, 1, 1, False),   # 384 x 192: the group kernel by default (the batched kernels of this shape,
+                                     # k_xinv_p<ZT> + k_ybracket_t with its v-fastest tile walk, run under kind 3 in
+                                     # test_spread_kernels_small_shapes_all_planes)
     # Nx = 768 with chi shared over v and Ny <= 192: k_xinv_p<768,...,ZT> + k_ybracket_t (on by default at these sizes)
     (512, 16, 2, 3, 1, 1, False), (512, 64, 1, 2, 1, 1, False),
-    (512, 128, 1, 2, 1, 1, False),   # the plane shape of configs[3]: k_xinv<768,...,SEQ> + k_ybracket<384> + k_xfwd<768>
-    (512, 128, 1, 1, 1, 1, True),
+    (512, 128, 1, 2, 1, 1, False),   # the plane shape of configs[3]: the group kernel (G = 8) by default; the batched kernels of
+                                     # this shape run in test_768x384_kernel_families
+    (512, 128, 1, 1, 1, 1, True),    # chi per plane at 768 x 384: batched (k_xinv<768,...,SEQ> + k_ybracket_cv<384> + k_xfwd<768>)
     # the wider size list (2^a 3^b): Nx = 288, 576, 1152, 1536 and Ny = 288, 576 (batched kernels)
     (192, 32, 2, 3, 1, 1, False), (192, 96, 1, 2, 1, 1, True),     # 288 x 96 (transposed-Z path), 288 x 288
     (384, 96, 1, 2, 1, 1, False), (32, 192, 2, 2, 1, 1, False),    # 576 x 288, 48 x 576
@@ -156,6 +159,7 @@ def test_errors_are_reported_not_swallowed(cuda_device):
 def _full_size(cuda_device, idx, nsample, plane_kernel=None):
     wl = W.CONFIGS[idx]
     need = 16 * wl.nx0 * wl.nky0 * (3 * wl.planes + wl.chi_planes) * 1.15
+    torch.cuda.empty_cache()       # blocks torch still caches from earlier tests are not "free" to the driver
     free, _ = torch.cuda.mem_get_info()
     if free < need:
         pytest.skip(f"{wl.name} needs {need / 2**30:.0f} GiB of device memory")
@@ -223,6 +227,33 @@ def test_spread_kernels_config2_full_size_all_planes(cuda_device, kind):
     _full_size(cuda_device, 2, None, plane_kernel=kind)
 
 
+# 768 x 384 planes (the shape of configs[3]): group kernel (2, the default), batched kernels (3: k_xinv<768,...,SEQ> +
+# k_ybracket<384> + k_xfwd<768>), warp-autonomous form (4).  40 planes > 2 x 18 groups of 8 CTAs, and the real-space chi
+# rows of the chunk (10 planes x 4.7 MB) exceed 40 MB, so that k_ybracket<384> takes its v-fastest tile walk under kind 3.
+@pytest.mark.parametrize("kind", [2, 3, 4])
+@pytest.mark.parametrize("nz,nv,nw,nspec", [(1, 1, 1, 1), (10, 4, 1, 1), (2, 3, 2, 2)])
+def test_768x384_kernel_families(cuda_device, nz, nv, nw, nspec, kind):
+    from paper_1310_1485_b200 import GeneNL
+    wl = W.small_workload(512, 128, nz, nv, nw, nspec, 0.0125, 0.025, False, seed=700 + nz + nv)
+    with GeneNL(wl, plane_kernel=kind) as nl:
+        assert (nl.query(7), nl.query(8)) == ((1.0, float(kind)) if kind != 3 else (0.0, 0.0))
+    with GeneNL(wl) as nl:
+        assert nl.query(8) == 2.0
+    check_parity(wl, cuda_device, plane_kernel=kind)
+    if nz * nv > 1:
+        check_parity(wl, cuda_device, plane_kernel=kind, scratch_bytes=40 << 20)   # several launches / ragged batches
+
+
+@pytest.mark.parametrize("kind", [3, 4])
+def test_config3_full_size_sampled_planes_other_kernel_families(cuda_device, kind):
+    """The full-size runs BASELINE.md quotes for the batched and the warp-autonomous kernels at configs[3]."""
+    _full_size(cuda_device, 3, 96, plane_kernel=kind)
+
+
+def test_config4_full_size_sampled_planes_warp_kernel(cuda_device):
+    _full_size(cuda_device, 4, 160, plane_kernel=4)
+
+
 @pytest.mark.parametrize("kind", SPREAD_KINDS)
 def test_spread_kernels_properties_and_selection(cuda_device, kind):
     from paper_1310_1485_b200 import (GENE_NL_KERNEL_AUTO, GENE_NL_KERNEL_BATCHED, GENE_NL_KERNEL_CLUSTER, GeneNL,
@@ -270,7 +301,8 @@ def test_spread_kernels_properties_and_selection(cuda_device, kind):
 # with chi shared over v, and the batched kernels on the same data
 @pytest.mark.parametrize("kind", [2, 3, 4])
 @pytest.mark.parametrize("chi_has_v", [True, False])
-@pytest.mark.parametrize("nz,nv,nw,nspec", [(1, 1, 1, 1), (3, 5, 2, 2), (37, 2, 1, 1)])
+@pytest.mark.parametrize("nz,nv,nw,nspec", [(1, 1, 1, 1), (3, 5, 2, 2), (37, 2, 1, 1),
+                                            (37, 9, 1, 1)])   # 333 planes > 2 x 148 groups: second and third plane per group
 def test_group_kernel_144x144_planes(cuda_device, nz, nv, nw, nspec, chi_has_v, kind):
     from paper_1310_1485_b200 import GeneNL
     wl = W.small_workload(96, 48, nz, nv, nw, nspec, 0.04, 0.06, chi_has_v, seed=400 + nz + nv)
@@ -285,26 +317,31 @@ def test_group_kernel_144x144_planes(cuda_device, nz, nv, nw, nspec, chi_has_v, 
     assert torch.equal(gpu_compute(wl, chi, g, rhs, scale=0.0, plane_kernel=kind), rhs)
 
 
-@pytest.mark.parametrize("nx0,nky0,chi_has_v,kind", [
-    (128, 32, False, None),      # k_plane_fused2: __syncwarp-only chains over in-place tiles, shadow lanes
-    (16, 8, False, None),        # k_plane_fused (first generation)
-    (256, 64, False, 2),         # k_plane_group: hand-overs through L2, counters, bulk copies into live tiles
-    (256, 64, False, 1),         # k_plane_cluster: DSMEM stores + mbarrier transaction counts
-    (96, 48, True, 2),           # k_plane_group with chi per plane (groups of one CTA)
-    (512, 128, False, 2),        # k_plane_group, radix-16 second y stage
-    (256, 64, True, 3),          # batched kernels
-    (256, 64, False, 4),         # k_plane_wa: per-warp tiles, every warp on the hand-over counters
-    (96, 48, True, 4),           # k_plane_wa with chi per plane
-    (512, 128, False, 4),        # k_plane_wa, radix-32 x stages
+# nw is chosen so that 3 * 5 * nw planes give every persistent CTA / cluster / group at least three planes (148 CTAs or
+# groups of one CTA: 450 planes; 37 groups of four: 120; 18 groups of eight and 15 clusters of eight: 60): the plane loop's
+# phase flips, the request of the next plane's first block and the dropped scratch lines are all exercised under
+# co-scheduling, not only a group's first plane
+@pytest.mark.parametrize("nx0,nky0,chi_has_v,kind,nw", [
+    (128, 32, False, None, 30),  # k_plane_fused2: __syncwarp-only chains over in-place tiles, shadow lanes
+    (16, 8, False, None, 30),    # k_plane_fused (first generation)
+    (256, 64, False, 2, 8),      # k_plane_group: hand-overs through L2, counters, bulk copies into live tiles
+    (256, 64, False, 1, 4),      # k_plane_cluster: DSMEM stores + mbarrier transaction counts
+    (96, 48, True, 2, 30),       # k_plane_group with chi per plane (groups of one CTA)
+    (96, 48, False, 2, 30),      # k_plane_group with chi shared over v (groups of one CTA)
+    (512, 128, False, 2, 4),     # k_plane_group, radix-16 second y stage
+    (256, 64, True, 3, 2),       # batched kernels
+    (256, 64, False, 4, 8),      # k_plane_wa: per-warp tiles, every warp on the hand-over counters
+    (96, 48, True, 4, 30),       # k_plane_wa with chi per plane
+    (512, 128, False, 4, 4),     # k_plane_wa, radix-32 x stages
 ])
-def test_repeated_runs_give_the_same_bits(cuda_device, nx0, nky0, chi_has_v, kind):
+def test_repeated_runs_give_the_same_bits(cuda_device, nx0, nky0, chi_has_v, kind, nw):
     """compute-sanitizer is closed on this pool (profiles/r02_sanitizer.md), so a data race in the shared-memory /
     distributed-shared-memory / L2 hand-overs has to show up here: the kernels are deterministic by construction (no
     atomics on data, fixed summation order), so 24 runs under different co-scheduling -- alone, behind a memory-bound
     kernel on another stream, with a different number of planes in flight -- must agree with the first one bit for bit,
     and that one with the oracle."""
     from paper_1310_1485_b200 import GeneNL
-    wl = W.small_workload(nx0, nky0, 3, 5, 2, 1, 0.04, 0.05, chi_has_v, seed=500 + nx0)
+    wl = W.small_workload(nx0, nky0, 3, 5, nw, 1, 0.04, 0.05, chi_has_v, seed=500 + nx0)
     chi, g, rhs = W.make_inputs(wl, cuda_device)
     check_parity(wl, cuda_device, plane_kernel=kind)
     junk = torch.empty(64 << 20, dtype=torch.float64, device=cuda_device)
@@ -321,7 +358,7 @@ def test_repeated_runs_give_the_same_bits(cuda_device, nx0, nky0, chi_has_v, kin
             nl.compute(chi, g, out)
             torch.cuda.synchronize()
             assert torch.equal(out, first), f"run {rep} differs"
-    half = W.small_workload(nx0, nky0, 3, 5, 1, 1, 0.04, 0.05, chi_has_v, seed=500 + nx0)   # first (w,s) slab only
+    half = W.small_workload(nx0, nky0, 3, 5, nw // 2, 1, 0.04, 0.05, chi_has_v, seed=500 + nx0)   # first half of the (w,s) slabs
     sub, cs, gs, rs = W.shard_arrays(wl, chi, g, rhs, 0, 2)
     assert sub.planes == half.planes
     part = gpu_compute(sub, cs.contiguous(), gs.contiguous(), rs.contiguous(), plane_kernel=kind)
