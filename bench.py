@@ -707,7 +707,8 @@ def run_config(wl, args, env, do_e2e, do_cpu, headline, plane_kernel=None):
                "h2d_bytes_per_step": 2 * gb + sub.plane_bytes * sub.chi_planes, "d2h_bytes_per_step": gb,
                "steps": args.e2e_steps,
                "api": "gene_nl_compute_host (pinned host buffers)" +
-                      ("" if ns == nslab else f" on the first {ns} of {nslab} (w,s) slabs = {sub.planes} planes per step")}
+                      ("" if ns == nslab else f" on the first {ns} of {nslab} (w,s) slabs = {sub.planes} planes per step") +
+                      "; bound by the host link (H2D of g, rhs and chi, D2H of rhs), not by the kernels (PAPER.md:115)"}
         del hchi, hg, hrhs
     else:
         del chi, g, rhs
