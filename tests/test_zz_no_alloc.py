@@ -62,6 +62,14 @@ def test_static_entry_point_matches_the_plan_path_on_two_calls_in_a_row(cuda_dev
     torch.cuda.synchronize()
     got, ref, r_in = _planes(out, wl), _planes(wants[1], wl), _planes(rhs, wl)
     assert plane_errors(wl, got, 2.0 * ref - r_in, r_in).max() <= TOL
+    # and the driver sees no allocation: free device memory is the same before and after further calls (the per-device
+    # set-up happened in the first call above; no torch allocation between the two readings)
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    for _ in range(3):
+        gene_nl_compute_static(wl.nx0, wl.nky0, wl.nz, wl.nv, wl.nw, wl.nspec, wl.kxmin, wl.kymin, chi, g, out, 0.0)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0
 
 
 def test_static_entry_point_rejects_what_its_scratch_was_not_laid_out_for():
