@@ -118,13 +118,23 @@ struct Grouped {
     static constexpr int TX_CPLX = UPP * CK * CSF;     // X2: exchange tiles of the units of one pass
     static constexpr int XR_CPLX = E_CPLX > TX_CPLX ? E_CPLX : TX_CPLX;
     static constexpr int G_CPLX = CK * NX0;            // one unit's columns of a spectral plane (one contiguous block)
-    // One region A serves the phases in turn: X1 (E at 0, the staged column block behind the x tiles), Y (the warps'
-    // pair storages: no block is in flight then), X2 (Tx at 0, the next plane's first block behind it).
-    static constexpr int GS_OFF = XR_CPLX;
-    static constexpr int A_CPLX = YB_CPLX > GS_OFF + G_CPLX ? YB_CPLX : GS_OFF + G_CPLX;
     static constexpr int TWX = AX * BPX, TWY = AY * BYP;
     static constexpr int TWX2 = (AX2 == AX && BX2 == BX) ? 0 : AX2 * BPX2;   // X2's own twiddle table when its split differs
     static constexpr int NBAR = 1 + NW;                // mbarriers: column block, rows of each warp
+    // With several k1 passes (NH > 1) the odd passes of X1 use a SECOND exchange tile E1 behind the first, so that the
+    // stores of pass hk + 1 need not wait for the stage-2 reads of pass hk: one CTA barrier per pass instead of two.  Its
+    // column-sign stride is the smallest odd one that holds AXH rows (the last row needs BX slots, not BPX).  Taken when
+    // the kernel still fits shared memory with the staged column block moved behind both tiles.
+    static constexpr int CSH1 = ((AXH - 1) * BPX + BX) | 1;
+    static constexpr int E1_OFF = E_CPLX;
+    static constexpr int E2_CPLX = E_CPLX + 2 * CK * CSH1;
+    static constexpr int GS_OFF_DB = XR_CPLX > E2_CPLX ? XR_CPLX : E2_CPLX;
+    static constexpr int A_CPLX_DB = YB_CPLX > GS_OFF_DB + G_CPLX ? YB_CPLX : GS_OFF_DB + G_CPLX;
+    static constexpr bool EDB = NH_ > 1 && sizeof(cplx) * (size_t)(A_CPLX_DB + TWX + TWX2 + TWY + (NBAR + 1) / 2) <= 227 * 1024;
+    // One region A serves the phases in turn: X1 (E at 0, E1 behind it, the staged column block behind the x tiles), Y (the
+    // warps' pair storages: no block is in flight then), X2 (Tx at 0, the next plane's first block behind it).
+    static constexpr int GS_OFF = EDB ? GS_OFF_DB : XR_CPLX;
+    static constexpr int A_CPLX = YB_CPLX > GS_OFF + G_CPLX ? YB_CPLX : GS_OFF + G_CPLX;
     static constexpr int SMEM_CPLX = A_CPLX + TWX + TWX2 + TWY + (NBAR + 1) / 2;
     static constexpr size_t SMEM_BYTES = sizeof(cplx) * (size_t)SMEM_CPLX;
     static constexpr int MINB = (NW <= 4 && SMEM_BYTES <= 113 * 1024) ? 2 : 1;   // CTAs per SM the kernel is built for
@@ -269,8 +279,10 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
             if (tid == 0 && s + 1 < NF * UPC) request_block(t, s + 1);
 #pragma unroll
             for (int hk = 0; hk < K::NH; ++hk) {
+                // odd passes go through the second tile when there is one (K::EDB)
+                const int eoff = (K::EDB && (hk & 1)) ? K::E1_OFF : 0, csh = (K::EDB && (hk & 1)) ? K::CSH1 : CSH;
                 if (has1) {
-                    cplx* Ec = A + c2 * CSH + n2;
+                    cplx* Ec = A + eoff + c2 * csh + n2;
 #pragma unroll
                     for (int k1 = 0; k1 < AXH; ++k1) Ec[k1 * BPX] = out[hk * AXH + k1];
                 }
@@ -282,7 +294,7 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     const int sg = c2s / CK, kyi = unit * CK + c2s % CK;
                     const bool zero = (sg == 1 && kyi == 0);  // there is no -0 column: slot cc = nky0 holds zeros
                     cplx v[BX];
-                    const cplx* Ec = A + c2s * CSH + (k1 - hk * AXH) * BPX;
+                    const cplx* Ec = A + eoff + c2s * csh + (k1 - hk * AXH) * BPX;
 #pragma unroll
                     for (int i = 0; i < BX; ++i) v[i] = zero ? cmake(0.0, 0.0) : Ec[i];
                     Dft<BX, +1>::run(v);
@@ -293,7 +305,9 @@ k_plane_group(const cplx* __restrict__ g, cplx* __restrict__ rhs, const cplx* __
                     for (int k2 = 0; k2 < BX; ++k2)      // pair storage: row m + NX/2 (k2 >= C2) first, then row m
                         stg_hint(Zc + (size_t)(AX * (k2 % C2)) * (2 * W2) + (k2 < C2 ? W2 : 0), cmake(v[k2].x, sgn * v[k2].y), pol_keep);
                 }
-                __syncthreads();  // E is free for the next k1 pass / the next step
+                // E is free for the next step (and, with one tile, for the next k1 pass).  With two tiles the barrier of
+                // pass hk + 1 already separates the stage-2 reads of pass hk from the stores of pass hk + 2 into the same tile.
+                if (!K::EDB || hk == K::NH - 1) __syncthreads();
             }
         }
         // ---- hand-over 1: every CTA of the group has written its columns of Z (a group of one: the CTA barrier that
